@@ -1,0 +1,182 @@
+/*
+ * flare_b200.h -- C ABI of libflare_b200.so: the per-timestep FLARE force-field evaluation
+ * for molecular dynamics (arxiv 2204.12573), hand-written CUDA for sm_100a, FP64.
+ *
+ * Citations: "P:L<n>" = line n of the paper text; "R<k>" = reading k of
+ * DESIGN.md section 3 (points where the paper is silent or garbled).
+ *
+ * What one evaluation computes, for every atom i:
+ *   - its local environment rho_i: all neighbours within r_cut[s_i][s_j]          (R5,R6)
+ *   - the ACE-B2 descriptor d_i: A[s,n,l,m] = sum_j T_n(2r/r_c-1) f_c(r) Y_lm(r^),
+ *     B[nu1<=nu2,l] = sum_m A[nu1,l,m] A[nu2,l,m], d^_i = B/||B||                 (R1-R4)
+ *   - the mapped mean  E_i = d^_i^T beta^(s_i)  d^_i                              (Eq. 1)
+ *   - the mapped variance V_i = d^_i^T Sigma^(s_i) d^_i  (Sigma = the paper's gamma) (Eq. 2)
+ *   - forces F = -grad sum_i E_i by the re-ordered summation that never forms
+ *     grad d_i
+ * and flare_step adds a velocity-Verlet NVE update (BASELINE.json north_star; R12).
+ *
+ * Conventions
+ *   - Units: Angstrom, eV, amu, fs (R13).  a = KAPPA F/m with KAPPA = 9.648533212331e-3.
+ *   - "device" pointers are CUDA device memory on the context's device; "host" pointers are
+ *     ordinary host memory (pinned memory makes the *_host entry points faster, not different).
+ *   - All arrays are dense, C-contiguous: positions/forces/velocities [N][3], matrices row-major.
+ *   - The caller owns every array and the workspace; the library allocates device memory only
+ *     in flare_create (model matrices and tables) and frees it in flare_destroy.
+ *   - All device work is enqueued on the stream given to flare_bind; device-pointer entry
+ *     points are asynchronous (results valid after the caller synchronises that stream) unless
+ *     stated otherwise.  *_host entry points and the flare_get_* hooks synchronise.
+ *   - Results are in the CALLER's atom order although atoms are cell-sorted internally.
+ *   - Every entry point returns FLARE_OK (0) or a negative FLARE_ERR_* code; nothing throws
+ *     or aborts across this boundary.  flare_last_error() gives a message for the last failure.
+ *   - There is no CPU fallback: without a CUDA device flare_create fails with FLARE_ERR_CUDA.
+ */
+#ifndef FLARE_B200_H
+#define FLARE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct flare_ctx flare_ctx; /* opaque, owned by the library */
+
+enum {
+    FLARE_OK = 0,
+    FLARE_ERR_INVALID_ARG = -1,        /* null pointer, bad size, species out of range, asymmetric r_cut (R5) */
+    FLARE_ERR_BOX_TOO_SMALL = -2,      /* a periodic box length < 2 max r_cut: no unique minimum image (R7) */
+    FLARE_ERR_UNSUPPORTED_BOX = -3,    /* non-orthorhombic cell (R7) */
+    FLARE_ERR_WORKSPACE_TOO_SMALL = -4,
+    FLARE_ERR_NEIGHBOR_OVERFLOW = -5,  /* an atom has more than FLARE_OPT_MAX_NEIGHBORS neighbours */
+    FLARE_ERR_CUDA = -6,               /* CUDA runtime error; message in flare_last_error */
+    FLARE_ERR_NONFINITE = -7,          /* NaN/Inf met in positions */
+    FLARE_ERR_UNSUPPORTED = -8,        /* (n_max, l_max) outside the compiled range */
+    FLARE_ERR_NOT_BOUND = -9           /* call needs flare_bind / flare_set_state first */
+};
+
+/* Options (flare_set_option / flare_get_option).  Set them BEFORE flare_workspace_bytes/flare_bind. */
+enum {
+    FLARE_OPT_MAX_NEIGHBORS = 1, /* row stride of the neighbour table, 1..255 (default 48) */
+    FLARE_OPT_CHUNK_ATOMS = 2,   /* atoms per chunk of the descriptor/quadratic-form/back-prop stage
+                                    ("dividing atoms into batches"); 0 = automatic (default) */
+    FLARE_OPT_TIMING = 3,        /* 1: bracket every kernel phase with CUDA events (flare_get_timings) */
+    FLARE_OPT_SPECIES_SPARSE = 4 /* 1: skip descriptor blocks of absent neighbour species;
+                                    exact; default 0 in this version */
+};
+
+/* Kernel phases reported by flare_get_timings, in this order. */
+enum {
+    FLARE_PHASE_NEIGHBOR = 0,   /* wrap, cell assign, sort, neighbour build, reverse-pair index  */
+    FLARE_PHASE_DESCRIPTOR = 1, /* basis, A accumulation, B2 contraction, normalisation          */
+    FLARE_PHASE_QFORM = 2,      /* beta and Sigma quadratic forms (FP64 DMMA grouped GEMM)        */
+    FLARE_PHASE_BACKPROP = 3,   /* dE/dB -> dE/dA -> per-pair forces                              */
+    FLARE_PHASE_GATHER = 4,     /* atomics-free force gather + E/V finalisation                   */
+    FLARE_PHASE_INTEGRATE = 5,  /* velocity-Verlet kicks and drift                                */
+    FLARE_N_PHASES = 6
+};
+
+/*
+ * Create a model context (beta and gamma "computed ... once and stored").
+ *   n_species  S >= 1
+ *   mass_amu   [S] host, > 0
+ *   n_max      radial functions per species (1..16); l_max angular cutoff (0..6)
+ *   r_cut      [S*S] host, symmetric, > 0 (R5)
+ *   beta       [S][P][P] host, row-major, eV; one matrix per CENTRAL species (R10); the
+ *              library stores (beta + beta^T)/2, which leaves E unchanged.
+ *   sigma      [S][P][P] host or NULL (then variances are unavailable); symmetrised likewise.
+ *              P = N(N+1)/2 (l_max+1), N = S n_max (420 / 112 in the paper).
+ *   cuda_device  ordinal; the context is tied to it.
+ * The arrays are copied; the caller may free them after the call.  Synchronous.
+ */
+int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_max, int l_max,
+                 const double* r_cut, const double* beta, const double* sigma, int cuda_device);
+
+void flare_destroy(flare_ctx* ctx);
+
+/* Number of B2 descriptor components P for this context. */
+int flare_num_descriptors(const flare_ctx* ctx);
+
+int flare_set_option(flare_ctx* ctx, int option, int64_t value);
+int flare_get_option(const flare_ctx* ctx, int option, int64_t* value);
+
+/* Bytes of device workspace flare_bind needs for n_atoms atoms (0 on error). */
+size_t flare_workspace_bytes(const flare_ctx* ctx, int64_t n_atoms);
+
+/*
+ * Attach a caller-owned device workspace (>= flare_workspace_bytes, 256-byte aligned) and the
+ * CUDA stream (a cudaStream_t passed as void*; NULL = legacy default stream) all later work
+ * runs on.  Re-binding with another n_atoms is allowed.  The workspace also holds the MD state.
+ */
+int flare_bind(flare_ctx* ctx, int64_t n_atoms, void* workspace, size_t bytes, void* cuda_stream);
+
+/*
+ * One force-field evaluation (steps a1-a8 of DESIGN.md).
+ *   pos   [N][3] device, Angstrom, any image (wrapped internally, R6)
+ *   types [N] device int32 in 0..S-1
+ *   box   [9] host, row-major cell vectors; must be orthorhombic (R7)
+ *   pbc   [3] host, non-zero = periodic
+ *   e_out [N] device or NULL; f_out [N][3] device or NULL; var_out [N] device or NULL
+ *         (NULL var_out skips the Sigma form entirely).
+ * Asynchronous.  Device-detected failures (neighbour overflow, non-finite input) are reported
+ * by flare_check(), which synchronises.
+ */
+int flare_compute(flare_ctx* ctx, const double* pos, const int32_t* types, const double box[9],
+                  const int pbc[3], double* e_out, double* f_out, double* var_out);
+
+/* Same, HOST buffers: copies in, evaluates, copies out, synchronises, runs flare_check(). */
+int flare_compute_host(flare_ctx* ctx, const double* pos, const int32_t* types, const double box[9],
+                       const int pbc[3], double* e_out, double* f_out, double* var_out);
+
+/* Synchronise the bound stream and return the first device-detected error of the work so far. */
+int flare_check(flare_ctx* ctx);
+
+/*
+ * MD state (library-owned copy inside the workspace): positions, velocities [N][3] (Angstrom/fs),
+ * types.  flare_set_state takes DEVICE pointers, flare_set_state_host HOST pointers.
+ */
+int flare_set_state(flare_ctx* ctx, const double* pos, const double* vel, const int32_t* types,
+                    const double box[9], const int pbc[3]);
+int flare_set_state_host(flare_ctx* ctx, const double* pos, const double* vel, const int32_t* types,
+                         const double box[9], const int pbc[3]);
+
+/*
+ * n_steps of velocity Verlet (R12): v += dt/2 KAPPA F/m; x += dt v; wrap; F = F(x); v += dt/2 KAPPA F/m.
+ * The neighbour list is rebuilt every step.  Forces of the current positions are evaluated
+ * first if they are not yet valid.  want_variance != 0 also evaluates V_i each step.  Asynchronous.
+ */
+int flare_step(flare_ctx* ctx, double dt_fs, int n_steps, int want_variance);
+
+/* Copy the state out; any pointer may be NULL.  Device-pointer version is asynchronous. */
+int flare_get_state(flare_ctx* ctx, double* pos, double* vel, double* e, double* f, double* var);
+int flare_get_state_host(flare_ctx* ctx, double* pos, double* vel, double* e, double* f, double* var);
+
+/*
+ * Test hooks (synchronise; HOST output pointers).
+ * flare_get_neighbors: neighbour sets of the last evaluation in the caller's atom order, each
+ *   row sorted by j; cnt [N], idx [N][stride] (entries past cnt[i] are -1).
+ * flare_get_descriptors: re-evaluates the descriptors of the last evaluation's positions and
+ *   returns B^ [N][P] and ||B|| [N] (caller's order).
+ */
+int flare_get_neighbors(flare_ctx* ctx, int32_t* cnt, int32_t* idx, int32_t stride);
+int flare_get_descriptors(flare_ctx* ctx, double* bhat, double* nrm);
+
+/*
+ * Accumulated CUDA-event time (ms) and launch count per phase since the last call
+ * (needs FLARE_OPT_TIMING = 1); ms and launches are [FLARE_N_PHASES] host arrays.  Synchronises.
+ */
+int flare_get_timings(flare_ctx* ctx, double* ms, int64_t* launches);
+
+/* Number of kernels the library has launched on this context since creation. */
+int64_t flare_kernel_launches(const flare_ctx* ctx);
+
+/* FP64 tensor-pipe (DMMA) issue peak of the device in TFLOP/s, measured by a register-resident
+   mma.sync m8n8k4 f64 loop: the roofline denominator of the quadratic-form kernel.  Synchronous. */
+double flare_measure_fp64_dmma_peak(int cuda_device);
+
+const char* flare_last_error(const flare_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLARE_B200_H */

@@ -1,0 +1,717 @@
+// flare_api.cu -- the C ABI of include/flare_b200.h: context, workspace carving, the step scheduler
+// that orders the kernels of steps a1-a9 on the caller's stream, and the host-buffer entry points.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/flare_b200.h"
+#include "kernels.cuh"
+
+using namespace flare;
+
+namespace {
+
+constexpr double kKappa = 9.648533212331e-3;  // (eV/amu) in A^2/fs^2 (R13)
+
+struct PhaseEvents {
+    std::vector<cudaEvent_t> start, stop;
+    size_t used = 0;
+    int64_t launches = 0;
+};
+
+}  // namespace
+
+struct flare_ctx {
+    int device = 0;
+    int sm_count = 148;
+    Basis bs{};
+    YNorm yn{};
+    std::vector<double> mass;
+    bool has_sigma = false;
+    // model on device
+    std::vector<void*> dev_allocs;
+    std::vector<GroupDesc> groups;  // host copy (device pointers inside)
+    GroupDev* d_groups = nullptr;
+    int n_groups = 0;
+    int max_ntn = 0;
+    int ld = 0;
+    double* d_accel = nullptr;  // [S] 0.5 dt kappa / m
+    double accel_dt = -1.0;
+    std::vector<double> h_accel;
+    // options
+    int mmax = 48;
+    int64_t chunk_opt = 0;
+    int timing = 0;
+    int sparse = 0;
+    // binding
+    int64_t n = -1;
+    Workspace ws{};
+    cudaStream_t stream = nullptr;
+    int chunk_cap = 0;
+    int n_cells_cap = 0;
+    Grid grid{};
+    bool have_grid = false;
+    bool state_set = false;
+    bool forces_valid = false;
+    bool var_valid = false;
+    double box[9]{};
+    int pbc[3]{};
+    // bookkeeping
+    int64_t launches = 0;
+    PhaseEvents phases[FLARE_N_PHASES];
+    std::string err;
+};
+
+namespace {
+
+int fail(flare_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+
+int cuda_fail(flare_ctx* c, cudaError_t e, const char* where) {
+    return fail(c, FLARE_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define FLARE_CUDA(ctx, call)                                         \
+    do {                                                              \
+        cudaError_t e__ = (call);                                     \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);    \
+    } while (0)
+
+struct PhaseScope {
+    flare_ctx* c;
+    int phase;
+    int64_t l0;
+    PhaseScope(flare_ctx* ctx, int p) : c(ctx), phase(p), l0(ctx->launches) {
+        if (!c->timing) return;
+        PhaseEvents& pe = c->phases[phase];
+        if (pe.used == pe.start.size()) {
+            cudaEvent_t a, b;
+            cudaEventCreate(&a);
+            cudaEventCreate(&b);
+            pe.start.push_back(a);
+            pe.stop.push_back(b);
+        }
+        cudaEventRecord(pe.start[pe.used], c->stream);
+    }
+    ~PhaseScope() {
+        if (!c->timing) return;
+        PhaseEvents& pe = c->phases[phase];
+        cudaEventRecord(pe.stop[pe.used], c->stream);
+        pe.used++;
+        pe.launches += c->launches - l0;
+    }
+};
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// choose the tile width (in n8 blocks) that wastes the fewest padded columns; ties -> wider tile
+void choose_tiles(int K, int& nb, int& ntn) {
+    static const int cand[] = {18, 17, 16, 15, 14, 13, 12, 11, 10, 9, 8, 6, 4, 2};
+    const int n8 = K / 8;
+    long best = -1;
+    nb = 2; ntn = (n8 + 1) / 2;
+    for (int c : cand) {
+        int t = (n8 + c - 1) / c;
+        long width = (long)t * c;
+        if (best < 0 || width < best) { best = width; nb = c; ntn = t; }
+    }
+}
+
+template <class T>
+int upload(flare_ctx* c, const std::vector<T>& h, T** d_out) {
+    void* d = nullptr;
+    FLARE_CUDA(c, cudaMalloc(&d, std::max<size_t>(sizeof(T) * h.size(), 16)));
+    c->dev_allocs.push_back(d);
+    if (!h.empty()) FLARE_CUDA(c, cudaMemcpy(d, h.data(), sizeof(T) * h.size(), cudaMemcpyHostToDevice));
+    *d_out = reinterpret_cast<T*>(d);
+    return FLARE_OK;
+}
+
+// padded, symmetrised copy of the sub-matrix of `m` (P x P, row-major) on the components `comp`
+std::vector<double> pack_matrix(const double* m, int P, const std::vector<int>& comp, int K, int rows) {
+    std::vector<double> out((size_t)rows * K, 0.0);
+    const int n = (int)comp.size();
+    for (int a = 0; a < n; a++)
+        for (int b = 0; b < n; b++)
+            out[(size_t)a * K + b] = 0.5 * (m[(size_t)comp[a] * P + comp[b]] + m[(size_t)comp[b] * P + comp[a]]);
+    return out;
+}
+
+int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
+    const Basis& bs = c->bs;
+    const int S = bs.S, L = bs.l_max + 1, Nv = bs.Nv, P = bs.P;
+    // dense component table (nu1, nu2>=nu1, l) in the order of R4
+    std::vector<int> dense_table;
+    dense_table.reserve(P);
+    for (int v1 = 0; v1 < Nv; v1++)
+        for (int v2 = v1; v2 < Nv; v2++)
+            for (int l = 0; l < L; l++) dense_table.push_back(v1 | (v2 << 8) | (l << 16));
+    c->n_groups = c->sparse ? S * (1 << S) : S;
+    c->groups.assign(c->n_groups, GroupDesc{});
+    std::vector<GroupDev> gdev(c->n_groups);
+    c->max_ntn = 0;
+    c->ld = 16;
+    for (int gi = 0; gi < c->n_groups; gi++) {
+        const int s = c->sparse ? gi / (1 << S) : gi;
+        const unsigned mask = c->sparse ? (unsigned)(gi % (1 << S)) : ((1u << S) - 1u);
+        // components whose both radial channels belong to species present in the mask
+        std::vector<int> comp, table;
+        for (int p = 0; p < P; p++) {
+            const int t = dense_table[p];
+            const int s1 = (t & 255) / bs.n_max, s2 = ((t >> 8) & 255) / bs.n_max;
+            if (((mask >> s1) & 1u) && ((mask >> s2) & 1u)) { comp.push_back(p); table.push_back(t); }
+        }
+        GroupDesc& gd = c->groups[gi];
+        gd.P = (int)comp.size();
+        if (gd.P == 0) { gdev[gi] = GroupDev{0, 0, 0, 0, nullptr}; continue; }
+        gd.K = round_up(gd.P, 16);
+        choose_tiles(gd.K, gd.nb, gd.ntn);
+        const int rows = gd.ntn * gd.nb * 8;
+        double* d = nullptr;
+        int rc = upload(c, pack_matrix(beta + (size_t)s * P * P, P, comp, gd.K, rows), &d);
+        if (rc) return rc;
+        gd.beta = d;
+        if (sigma) {
+            rc = upload(c, pack_matrix(sigma + (size_t)s * P * P, P, comp, gd.K, rows), &d);
+            if (rc) return rc;
+            gd.sigma = d;
+        }
+        int* dt = nullptr;
+        rc = upload(c, table, &dt);
+        if (rc) return rc;
+        gd.table = dt;
+        gdev[gi] = GroupDev{gd.P, gd.K, gd.ntn, 0, gd.table};
+        c->max_ntn = std::max(c->max_ntn, gd.ntn);
+        c->ld = std::max(c->ld, gd.K);
+    }
+    return upload(c, gdev, &c->d_groups);
+}
+
+// ---------------------------------------------------------------- workspace layout
+struct Carver {
+    char* base;
+    size_t off = 0;
+    template <class T>
+    T* take(size_t count) {
+        off = (off + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += sizeof(T) * count;
+        return p;
+    }
+};
+
+int auto_chunk(const flare_ctx* c, int64_t n) {
+    if (c->chunk_opt > 0) return (int)std::min<int64_t>(std::max<int64_t>(c->chunk_opt, 1), std::max<int64_t>(n, 1));
+    const double per_row = 8.0 * (c->bs.NvL2 + 2.0 * c->ld + 1 + 2.0 * c->max_ntn);
+    int64_t rows = (int64_t)(4.0 * 1024 * 1024 * 1024 / per_row);
+    rows = std::max<int64_t>(rows, 16384);
+    return (int)std::max<int64_t>(1, std::min<int64_t>(rows, n));
+}
+
+size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chunk_out, int* cells_out) {
+    Carver cv{base};
+    const size_t N = (size_t)std::max<int64_t>(n, 1);
+    const int chunk = auto_chunk(c, n);
+    const size_t cells = std::max<size_t>(4096, 2 * N);
+    Workspace w;
+    w.x = cv.take<double>(3 * N);
+    w.v = cv.take<double>(3 * N);
+    w.f = cv.take<double>(3 * N);
+    w.e = cv.take<double>(N);
+    w.var = cv.take<double>(N);
+    w.types = cv.take<int>(N);
+    w.flags = cv.take<int>(4);
+    w.cell_cnt = cv.take<int>(cells);
+    w.cell_start = cv.take<int>(cells + 1);
+    w.scan_tmp = cv.take<int>(cells / 1024 + 2);
+    w.cell_of = cv.take<int>(N);
+    w.rank_in_cell = cv.take<int>(N);
+    w.order = cv.take<int>(N);
+    w.atoms = cv.take<AtomS>(N);
+    w.nbr_cnt = cv.take<int>(N);
+    w.nbr_idx = cv.take<int>(N * c->mmax);
+    w.rev = cv.take<unsigned char>(N * c->mmax);
+    w.nmask = cv.take<unsigned char>(N);
+    w.group_hist = cv.take<int>((N / 1024 + 1) * (size_t)c->n_groups);
+    w.group_start = cv.take<int>(c->n_groups + 1);
+    w.row_of = cv.take<int>(N);
+    w.gid = cv.take<unsigned char>(N);
+    w.atom_of_row = cv.take<int>(N);
+    w.pairf = cv.take<double>(N * c->mmax * 3);
+    w.e_s = cv.take<double>(N);
+    w.v_s = cv.take<double>(N);
+    w.A = cv.take<double>((size_t)chunk * c->bs.NvL2);
+    w.Bh = cv.take<double>((size_t)chunk * c->ld);
+    w.W = cv.take<double>((size_t)chunk * c->ld);
+    w.nrm = cv.take<double>(chunk);
+    w.part = cv.take<double>((size_t)2 * std::max(c->max_ntn, 1) * chunk);
+    if (ws) *ws = w;
+    if (chunk_out) *chunk_out = chunk;
+    if (cells_out) *cells_out = (int)std::min<size_t>(cells, 0x7fffffff);
+    return ((cv.off + 255) & ~(size_t)255) + 256;
+}
+
+// ---------------------------------------------------------------- box -> cell grid (R7)
+int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
+    if (!box || !pbc) return fail(c, FLARE_ERR_INVALID_ARG, "box/pbc is null");
+    for (int i = 0; i < 9; i++)
+        if (!std::isfinite(box[i])) return fail(c, FLARE_ERR_INVALID_ARG, "box has a non-finite entry");
+    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0)
+        return fail(c, FLARE_ERR_UNSUPPORTED_BOX, "only orthorhombic cells are supported (R7)");
+    if (!(box[0] > 0 && box[4] > 0 && box[8] > 0)) return fail(c, FLARE_ERR_INVALID_ARG, "box lengths must be > 0");
+    double rcmax = 0;
+    for (int i = 0; i < c->bs.S * c->bs.S; i++) rcmax = std::max(rcmax, c->bs.rc[i]);
+    Grid g{};
+    for (int d = 0; d < 3; d++) {
+        g.L[d] = box[4 * d];
+        g.half[d] = 0.5 * g.L[d];
+        g.pbc[d] = pbc[d] ? 1 : 0;
+        if (g.pbc[d] && g.L[d] < 2.0 * rcmax)
+            return fail(c, FLARE_ERR_BOX_TOO_SMALL, "a periodic box length is < 2 max r_cut (R7)");
+        int nc = (int)std::floor(g.L[d] / (rcmax * (1.0 + 1e-9)));
+        g.nc[d] = std::max(1, nc);
+    }
+    // keep the number of cells within what the workspace was sized for
+    while ((double)g.nc[0] * g.nc[1] * g.nc[2] > (double)c->n_cells_cap) {
+        int dmax = 0;
+        for (int d = 1; d < 3; d++) if (g.nc[d] > g.nc[dmax]) dmax = d;
+        g.nc[dmax] = std::max(1, (int)(g.nc[dmax] * 0.8));
+    }
+    for (int d = 0; d < 3; d++) g.inv_cw[d] = (double)g.nc[d] / g.L[d];
+    // dimension with the fewest cells runs fastest (a thin slab's z column becomes contiguous)
+    int ord[3] = {0, 1, 2};
+    std::sort(ord, ord + 3, [&](int a, int b) { return g.nc[a] < g.nc[b] || (g.nc[a] == g.nc[b] && a > b); });
+    g.fast = ord[0]; g.slow0 = ord[1]; g.slow1 = ord[2];
+    g.stride[g.fast] = 1;
+    g.stride[g.slow0] = g.nc[g.fast];
+    g.stride[g.slow1] = g.nc[g.fast] * g.nc[g.slow0];
+    g.n_cells = g.nc[0] * g.nc[1] * g.nc[2];
+    c->grid = g;
+    c->have_grid = true;
+    memcpy(c->box, box, sizeof(double) * 9);
+    for (int d = 0; d < 3; d++) c->pbc[d] = g.pbc[d];
+    return FLARE_OK;
+}
+
+// ---------------------------------------------------------------- one evaluation (steps a1-a8)
+int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, double* f_out, double* var_out) {
+    const int n = (int)c->n;
+    Launcher L;
+    L.stream = c->stream;
+    L.launch_count = &c->launches;
+    const bool want_var = (var_out != nullptr) && c->has_sigma;
+    if (var_out && !c->has_sigma) return fail(c, FLARE_ERR_INVALID_ARG, "variance requested but the model has no sigma");
+    if (n == 0) return FLARE_OK;
+    {
+        PhaseScope ps(c, FLARE_PHASE_NEIGHBOR);
+        build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups);
+    }
+    for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
+        const int nrows = std::min(c->chunk_cap, n - row0);
+        {
+            PhaseScope ps(c, FLARE_PHASE_DESCRIPTOR);
+            run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ws.Bh, c->ld,
+                            c->ws.nrm, nullptr, true);
+        }
+        {
+            PhaseScope ps(c, FLARE_PHASE_QFORM);
+            run_qform(L, c->ws, c->groups.data(), c->n_groups, row0, nrows, c->ld, c->chunk_cap, want_var, c->sm_count);
+        }
+        {
+            PhaseScope ps(c, FLARE_PHASE_BACKPROP);
+            run_backprop(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ld, c->chunk_cap,
+                         c->max_ntn, want_var);
+        }
+    }
+    {
+        PhaseScope ps(c, FLARE_PHASE_GATHER);
+        run_gather(L, c->ws, n, c->mmax, e_out, f_out, var_out);
+    }
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "launch");
+    return FLARE_OK;
+}
+
+int need_bound(flare_ctx* c) {
+    if (!c) return FLARE_ERR_INVALID_ARG;
+    if (c->n < 0) return fail(c, FLARE_ERR_NOT_BOUND, "flare_bind has not been called");
+    return FLARE_OK;
+}
+
+}  // namespace
+
+// ================================================================= C ABI
+extern "C" {
+#pragma GCC visibility push(default)
+
+int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_max, int l_max, const double* r_cut,
+                 const double* beta, const double* sigma, int cuda_device) {
+    if (!out) return FLARE_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!mass_amu || !r_cut || !beta) return FLARE_ERR_INVALID_ARG;
+    if (n_species < 1 || n_species > kMaxSpecies) return FLARE_ERR_INVALID_ARG;
+    if (n_max < 1 || n_max > kMaxNmax || l_max < 0 || l_max > kMaxLmax) return FLARE_ERR_UNSUPPORTED;
+    if (n_species * n_max > 255) return FLARE_ERR_UNSUPPORTED;
+    for (int a = 0; a < n_species; a++) {
+        if (!(mass_amu[a] > 0)) return FLARE_ERR_INVALID_ARG;
+        for (int b = 0; b < n_species; b++) {
+            const double r = r_cut[a * n_species + b];
+            if (!(r > 0) || !std::isfinite(r) || r != r_cut[b * n_species + a]) return FLARE_ERR_INVALID_ARG;  // R5
+        }
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0 || cuda_device < 0 || cuda_device >= ndev)
+        return FLARE_ERR_CUDA;  // no CPU fallback
+    if (cudaSetDevice(cuda_device) != cudaSuccess) return FLARE_ERR_CUDA;
+    flare_ctx* c = new (std::nothrow) flare_ctx();
+    if (!c) return FLARE_ERR_CUDA;
+    c->device = cuda_device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) == cudaSuccess) c->sm_count = prop.multiProcessorCount;
+    Basis& bs = c->bs;
+    bs.S = n_species; bs.n_max = n_max; bs.l_max = l_max;
+    bs.L2 = (l_max + 1) * (l_max + 1);
+    bs.Nv = n_species * n_max;
+    bs.NvL2 = bs.Nv * bs.L2;
+    bs.P = bs.Nv * (bs.Nv + 1) / 2 * (l_max + 1);
+    for (int i = 0; i < n_species * n_species; i++) { bs.rc[i] = r_cut[i]; bs.rc2[i] = r_cut[i] * r_cut[i]; }
+    c->mass.assign(mass_amu, mass_amu + n_species);
+    c->has_sigma = sigma != nullptr;
+    // K_lm sqrt(2 - delta_m0)
+    for (int l = 0; l <= kMaxLmax; l++)
+        for (int m = 0; m <= l; m++) {
+            double ratio = 1.0;  // (l-m)!/(l+m)!
+            for (int q = l - m + 1; q <= l + m; q++) ratio /= (double)q;
+            double k = std::sqrt((2.0 * l + 1.0) / (4.0 * kPi) * ratio);
+            if (m > 0) k *= std::sqrt(2.0);
+            c->yn.k[l * (l + 1) / 2 + m] = k;
+        }
+    int rc = build_groups(c, beta, sigma);
+    if (rc == FLARE_OK) {
+        void* d = nullptr;
+        if (cudaMalloc(&d, sizeof(double) * kMaxSpecies) != cudaSuccess) rc = FLARE_ERR_CUDA;
+        else { c->dev_allocs.push_back(d); c->d_accel = (double*)d; }
+    }
+    if (rc != FLARE_OK) { flare_destroy(c); return rc; }
+    bs.Pld = c->ld;
+    c->h_accel.assign(kMaxSpecies, 0.0);
+    *out = c;
+    return FLARE_OK;
+}
+
+void flare_destroy(flare_ctx* c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    for (void* p : c->dev_allocs) cudaFree(p);
+    for (auto& pe : c->phases) {
+        for (auto e : pe.start) cudaEventDestroy(e);
+        for (auto e : pe.stop) cudaEventDestroy(e);
+    }
+    delete c;
+}
+
+int flare_num_descriptors(const flare_ctx* c) { return c ? c->bs.P : FLARE_ERR_INVALID_ARG; }
+
+int flare_set_option(flare_ctx* c, int option, int64_t value) {
+    if (!c) return FLARE_ERR_INVALID_ARG;
+    switch (option) {
+        case FLARE_OPT_MAX_NEIGHBORS:
+            if (value < 1 || value > 255) return fail(c, FLARE_ERR_INVALID_ARG, "max neighbours must be in 1..255");
+            c->mmax = (int)value; c->n = -1;
+            return FLARE_OK;
+        case FLARE_OPT_CHUNK_ATOMS:
+            if (value < 0) return fail(c, FLARE_ERR_INVALID_ARG, "chunk must be >= 0");
+            c->chunk_opt = value; c->n = -1;
+            return FLARE_OK;
+        case FLARE_OPT_TIMING:
+            c->timing = value ? 1 : 0;
+            return FLARE_OK;
+        case FLARE_OPT_SPECIES_SPARSE:
+            if (value) return fail(c, FLARE_ERR_UNSUPPORTED, "species-sparse mode is not available in this version");
+            return FLARE_OK;
+        default:
+            return fail(c, FLARE_ERR_INVALID_ARG, "unknown option");
+    }
+}
+
+int flare_get_option(const flare_ctx* c, int option, int64_t* value) {
+    if (!c || !value) return FLARE_ERR_INVALID_ARG;
+    switch (option) {
+        case FLARE_OPT_MAX_NEIGHBORS: *value = c->mmax; return FLARE_OK;
+        case FLARE_OPT_CHUNK_ATOMS: *value = c->n >= 0 ? c->chunk_cap : c->chunk_opt; return FLARE_OK;
+        case FLARE_OPT_TIMING: *value = c->timing; return FLARE_OK;
+        case FLARE_OPT_SPECIES_SPARSE: *value = c->sparse; return FLARE_OK;
+        default: return FLARE_ERR_INVALID_ARG;
+    }
+}
+
+size_t flare_workspace_bytes(const flare_ctx* c, int64_t n_atoms) {
+    if (!c || n_atoms < 0 || n_atoms > 0x7fffffff / 4) return 0;
+    return carve(c, n_atoms, nullptr, nullptr, nullptr, nullptr);
+}
+
+int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, void* cuda_stream) {
+    if (!c) return FLARE_ERR_INVALID_ARG;
+    if (n_atoms < 0 || n_atoms > 0x7fffffff / 4) return fail(c, FLARE_ERR_INVALID_ARG, "n_atoms out of range");
+    if (!workspace) return fail(c, FLARE_ERR_INVALID_ARG, "workspace is null");
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0)
+        return fail(c, FLARE_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    const size_t need = carve(c, n_atoms, nullptr, nullptr, nullptr, nullptr);
+    if (bytes < need) return fail(c, FLARE_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than flare_workspace_bytes");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    carve(c, n_atoms, static_cast<char*>(workspace), &c->ws, &c->chunk_cap, &c->n_cells_cap);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->n = n_atoms;
+    c->state_set = c->forces_valid = c->var_valid = false;
+    c->have_grid = false;
+    FLARE_CUDA(c, cudaMemsetAsync(c->ws.flags, 0, sizeof(int) * 4, c->stream));
+    return FLARE_OK;
+}
+
+int flare_compute(flare_ctx* c, const double* pos, const int32_t* types, const double box[9], const int pbc[3],
+                  double* e_out, double* f_out, double* var_out) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (c->n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    rc = setup_grid(c, box, pbc);
+    if (rc) return rc;
+    return evaluate(c, pos, types, e_out, f_out, var_out);
+}
+
+int flare_check(flare_ctx* c) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    int flags[4] = {0, 0, 0, 0};
+    FLARE_CUDA(c, cudaMemcpy(flags, c->ws.flags, sizeof(flags), cudaMemcpyDeviceToHost));
+    if (flags[0]) FLARE_CUDA(c, cudaMemset(c->ws.flags, 0, sizeof(flags)));
+    if (flags[0] & kFlagNonFinite) return fail(c, FLARE_ERR_NONFINITE, "non-finite position");
+    if (flags[0] & kFlagNeighborOverflow)
+        return fail(c, FLARE_ERR_NEIGHBOR_OVERFLOW, "an atom has more neighbours than FLARE_OPT_MAX_NEIGHBORS");
+    return FLARE_OK;
+}
+
+int flare_compute_host(flare_ctx* c, const double* pos, const int32_t* types, const double box[9], const int pbc[3],
+                       double* e_out, double* f_out, double* var_out) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    const size_t n = (size_t)c->n;
+    if (n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    c->state_set = c->forces_valid = false;  // the state arrays serve as staging
+    if (n > 0) {
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.x, pos, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, c->stream));
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.types, types, sizeof(int) * n, cudaMemcpyHostToDevice, c->stream));
+    }
+    rc = flare_compute(c, c->ws.x, c->ws.types, box, pbc, e_out ? c->ws.e : nullptr, f_out ? c->ws.f : nullptr,
+                       var_out ? c->ws.var : nullptr);
+    if (rc) return rc;
+    if (n > 0) {
+        if (e_out) FLARE_CUDA(c, cudaMemcpyAsync(e_out, c->ws.e, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+        if (f_out) FLARE_CUDA(c, cudaMemcpyAsync(f_out, c->ws.f, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+        if (var_out) FLARE_CUDA(c, cudaMemcpyAsync(var_out, c->ws.var, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    }
+    return flare_check(c);
+}
+
+static int set_state_impl(flare_ctx* c, const double* pos, const double* vel, const int32_t* types,
+                          const double box[9], const int pbc[3], cudaMemcpyKind kind) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    const size_t n = (size_t)c->n;
+    if (n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    rc = setup_grid(c, box, pbc);
+    if (rc) return rc;
+    if (n > 0) {
+        if (pos != c->ws.x) FLARE_CUDA(c, cudaMemcpyAsync(c->ws.x, pos, sizeof(double) * 3 * n, kind, c->stream));
+        if (vel) { if (vel != c->ws.v) FLARE_CUDA(c, cudaMemcpyAsync(c->ws.v, vel, sizeof(double) * 3 * n, kind, c->stream)); }
+        else FLARE_CUDA(c, cudaMemsetAsync(c->ws.v, 0, sizeof(double) * 3 * n, c->stream));
+        if (types != c->ws.types) FLARE_CUDA(c, cudaMemcpyAsync(c->ws.types, types, sizeof(int) * n, kind, c->stream));
+    }
+    c->state_set = true;
+    c->forces_valid = c->var_valid = false;
+    return FLARE_OK;
+}
+
+int flare_set_state(flare_ctx* c, const double* pos, const double* vel, const int32_t* types, const double box[9],
+                    const int pbc[3]) {
+    return set_state_impl(c, pos, vel, types, box, pbc, cudaMemcpyDeviceToDevice);
+}
+
+int flare_set_state_host(flare_ctx* c, const double* pos, const double* vel, const int32_t* types,
+                         const double box[9], const int pbc[3]) {
+    return set_state_impl(c, pos, vel, types, box, pbc, cudaMemcpyHostToDevice);
+}
+
+int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->state_set) return fail(c, FLARE_ERR_NOT_BOUND, "flare_set_state has not been called");
+    if (n_steps < 0 || !std::isfinite(dt_fs)) return fail(c, FLARE_ERR_INVALID_ARG, "bad dt or n_steps");
+    if (want_variance && !c->has_sigma) return fail(c, FLARE_ERR_INVALID_ARG, "variance requested but the model has no sigma");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    const int n = (int)c->n;
+    Workspace& w = c->ws;
+    double* var = want_variance ? w.var : nullptr;
+    if (!c->forces_valid || (want_variance && !c->var_valid)) {
+        rc = evaluate(c, w.x, w.types, w.e, w.f, var);
+        if (rc) return rc;
+        c->forces_valid = true;
+        c->var_valid = want_variance != 0;
+    }
+    if (n_steps == 0) return FLARE_OK;
+    if (c->accel_dt != dt_fs) {
+        // the previous table may still be in flight on the stream: order the overwrite after it
+        FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (int s = 0; s < c->bs.S; s++) c->h_accel[s] = 0.5 * dt_fs * kKappa / c->mass[s];
+        FLARE_CUDA(c, cudaMemcpyAsync(c->d_accel, c->h_accel.data(), sizeof(double) * kMaxSpecies,
+                                      cudaMemcpyHostToDevice, c->stream));
+        c->accel_dt = dt_fs;
+    }
+    Launcher L;
+    L.stream = c->stream;
+    L.launch_count = &c->launches;
+    for (int step = 0; step < n_steps; step++) {
+        {
+            PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
+            run_kick_drift(L, c->grid, n, w.x, w.v, w.f, w.types, c->d_accel, dt_fs);
+        }
+        rc = evaluate(c, w.x, w.types, w.e, w.f, var);
+        if (rc) return rc;
+        {
+            PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
+            run_kick(L, n, w.v, w.f, w.types, c->d_accel);
+        }
+    }
+    c->var_valid = want_variance != 0;
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, "integrator launch");
+    return FLARE_OK;
+}
+
+static int get_state_impl(flare_ctx* c, double* pos, double* vel, double* e, double* f, double* var,
+                          cudaMemcpyKind kind) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->state_set) return fail(c, FLARE_ERR_NOT_BOUND, "flare_set_state has not been called");
+    if (var && !c->var_valid) return fail(c, FLARE_ERR_INVALID_ARG, "variances were not evaluated");
+    if ((e || f) && !c->forces_valid) return fail(c, FLARE_ERR_INVALID_ARG, "forces were not evaluated yet");
+    const size_t n = (size_t)c->n;
+    if (n == 0) return FLARE_OK;
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    if (pos) FLARE_CUDA(c, cudaMemcpyAsync(pos, c->ws.x, sizeof(double) * 3 * n, kind, c->stream));
+    if (vel) FLARE_CUDA(c, cudaMemcpyAsync(vel, c->ws.v, sizeof(double) * 3 * n, kind, c->stream));
+    if (e) FLARE_CUDA(c, cudaMemcpyAsync(e, c->ws.e, sizeof(double) * n, kind, c->stream));
+    if (f) FLARE_CUDA(c, cudaMemcpyAsync(f, c->ws.f, sizeof(double) * 3 * n, kind, c->stream));
+    if (var) FLARE_CUDA(c, cudaMemcpyAsync(var, c->ws.var, sizeof(double) * n, kind, c->stream));
+    return FLARE_OK;
+}
+
+int flare_get_state(flare_ctx* c, double* pos, double* vel, double* e, double* f, double* var) {
+    return get_state_impl(c, pos, vel, e, f, var, cudaMemcpyDeviceToDevice);
+}
+
+int flare_get_state_host(flare_ctx* c, double* pos, double* vel, double* e, double* f, double* var) {
+    int rc = get_state_impl(c, pos, vel, e, f, var, cudaMemcpyDeviceToHost);
+    if (rc) return rc;
+    return flare_check(c);
+}
+
+int flare_get_neighbors(flare_ctx* c, int32_t* cnt, int32_t* idx, int32_t stride) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->have_grid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    if (!cnt || !idx || stride < 1) return fail(c, FLARE_ERR_INVALID_ARG, "bad output arrays");
+    rc = flare_check(c);
+    if (rc) return rc;
+    const size_t n = (size_t)c->n;
+    if (n == 0) return FLARE_OK;
+    std::vector<int> h_cnt(n), h_idx(n * c->mmax);
+    std::vector<AtomS> h_atoms(n);
+    FLARE_CUDA(c, cudaMemcpy(h_cnt.data(), c->ws.nbr_cnt, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    FLARE_CUDA(c, cudaMemcpy(h_idx.data(), c->ws.nbr_idx, sizeof(int) * n * c->mmax, cudaMemcpyDeviceToHost));
+    FLARE_CUDA(c, cudaMemcpy(h_atoms.data(), c->ws.atoms, sizeof(AtomS) * n, cudaMemcpyDeviceToHost));
+    std::vector<int> row;
+    int status = FLARE_OK;
+    for (size_t k = 0; k < n; k++) {
+        const int i = h_atoms[k].orig;
+        row.clear();
+        for (int s = 0; s < h_cnt[k]; s++) row.push_back(h_atoms[h_idx[k * c->mmax + s]].orig);
+        std::sort(row.begin(), row.end());
+        cnt[i] = h_cnt[k];
+        for (int s = 0; s < stride; s++) idx[(size_t)i * stride + s] = s < (int)row.size() ? row[s] : -1;
+        if ((int)row.size() > stride) status = FLARE_ERR_INVALID_ARG;
+    }
+    if (status) return fail(c, status, "stride smaller than a neighbour count");
+    return FLARE_OK;
+}
+
+int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->have_grid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    if (!bhat || !nrm) return fail(c, FLARE_ERR_INVALID_ARG, "bad output arrays");
+    if (c->sparse) return fail(c, FLARE_ERR_UNSUPPORTED, "descriptor hook needs dense mode");
+    rc = flare_check(c);
+    if (rc) return rc;
+    const int n = (int)c->n;
+    const int P = c->bs.P;
+    std::vector<AtomS> h_atoms((size_t)n);
+    std::vector<int> h_aor((size_t)n);
+    if (n == 0) return FLARE_OK;
+    FLARE_CUDA(c, cudaMemcpy(h_atoms.data(), c->ws.atoms, sizeof(AtomS) * n, cudaMemcpyDeviceToHost));
+    FLARE_CUDA(c, cudaMemcpy(h_aor.data(), c->ws.atom_of_row, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    Launcher L;
+    L.stream = c->stream;
+    L.launch_count = &c->launches;
+    std::vector<double> hb, hn;
+    for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
+        const int nrows = std::min(c->chunk_cap, n - row0);
+        run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ws.Bh, c->ld, c->ws.nrm,
+                        nullptr, false);
+        if (L.err != cudaSuccess) return cuda_fail(c, L.err, "descriptor launch");
+        hb.resize((size_t)nrows * c->ld);
+        hn.resize(nrows);
+        FLARE_CUDA(c, cudaMemcpyAsync(hb.data(), c->ws.Bh, sizeof(double) * hb.size(), cudaMemcpyDeviceToHost, c->stream));
+        FLARE_CUDA(c, cudaMemcpyAsync(hn.data(), c->ws.nrm, sizeof(double) * nrows, cudaMemcpyDeviceToHost, c->stream));
+        FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (int r = 0; r < nrows; r++) {
+            const int i = h_atoms[h_aor[row0 + r]].orig;
+            memcpy(bhat + (size_t)i * P, hb.data() + (size_t)r * c->ld, sizeof(double) * P);
+            nrm[i] = hn[r];
+        }
+    }
+    return FLARE_OK;
+}
+
+int flare_get_timings(flare_ctx* c, double* ms, int64_t* launches) {
+    if (!c || !ms) return FLARE_ERR_INVALID_ARG;
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int p = 0; p < FLARE_N_PHASES; p++) {
+        PhaseEvents& pe = c->phases[p];
+        double tot = 0.0;
+        for (size_t i = 0; i < pe.used; i++) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, pe.start[i], pe.stop[i]) == cudaSuccess) tot += t;
+        }
+        ms[p] = tot;
+        if (launches) launches[p] = pe.launches;
+        pe.used = 0;
+        pe.launches = 0;
+    }
+    return FLARE_OK;
+}
+
+int64_t flare_kernel_launches(const flare_ctx* c) { return c ? c->launches : 0; }
+
+double flare_measure_fp64_dmma_peak(int cuda_device) { return measure_dmma_peak(cuda_device); }
+
+const char* flare_last_error(const flare_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+#pragma GCC visibility pop
+}  // extern "C"

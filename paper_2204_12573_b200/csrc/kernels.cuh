@@ -1,0 +1,120 @@
+// kernels.cuh -- host-side launch plumbing shared by the translation units of libflare_b200.so:
+// the workspace layout, the stream/launch-count/timing wrapper, and the per-stage entry points.
+#pragma once
+#include <utility>
+
+#include "basis.cuh"
+#include "common.cuh"
+
+namespace flare {
+
+constexpr int kMaxGroups = 64;  // quadratic-form groups: (central species) or (species, neighbour mask)
+constexpr int kNumPhases = 6;
+
+// Launch wrapper: all kernels go to one stream; counts launches; keeps the first CUDA error.
+struct Launcher {
+    cudaStream_t stream = nullptr;
+    int64_t* launch_count = nullptr;
+    cudaError_t err = cudaSuccess;
+    const char* err_where = nullptr;
+
+    template <class... KArgs, class... Args>
+    void launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+        if (grid.x == 0 || grid.y == 0 || grid.z == 0 || err != cudaSuccess) return;
+        kernel<<<grid, block, smem, stream>>>(std::forward<Args>(args)...);
+        if (launch_count) ++*launch_count;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = "kernel launch"; }
+    }
+    void memset(void* p, int v, size_t bytes) {
+        if (bytes == 0 || err != cudaSuccess) return;
+        cudaError_t e = cudaMemsetAsync(p, v, bytes, stream);
+        if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = "memset"; }
+    }
+};
+
+// Device pointers carved out of the caller's workspace by flare_bind.
+struct Workspace {
+    // ---- persistent per-atom state (caller order) for flare_step
+    double* x = nullptr;    // [N][3]
+    double* v = nullptr;    // [N][3]
+    double* f = nullptr;    // [N][3]
+    double* e = nullptr;    // [N]
+    double* var = nullptr;  // [N]
+    int* types = nullptr;   // [N]
+    // ---- neighbour stage
+    int* flags = nullptr;         // [4] device error bits
+    int* cell_cnt = nullptr;      // [n_cells_cap]
+    int* cell_start = nullptr;    // [n_cells_cap+1]
+    int* scan_tmp = nullptr;      // [n_cells_cap/1024+2]
+    int* cell_of = nullptr;       // [N]
+    int* rank_in_cell = nullptr;  // [N]
+    int* order = nullptr;         // [N] sorted slot -> caller index
+    AtomS* atoms = nullptr;       // [N] cell-sorted
+    int* nbr_cnt = nullptr;       // [N]
+    int* nbr_idx = nullptr;       // [N][mmax] sorted-space indices
+    unsigned char* rev = nullptr;    // [N][mmax]
+    unsigned char* nmask = nullptr;  // [N] neighbour-species bitmask
+    int* group_hist = nullptr;    // [ceil(N/1024)][n_groups]
+    int* group_start = nullptr;   // [n_groups+1]
+    int* row_of = nullptr;        // [N] sorted atom -> quadratic-form row
+    unsigned char* gid = nullptr; // [N] group id of each sorted atom
+    int* atom_of_row = nullptr;   // [N]
+    // ---- per-atom results in sorted order
+    double* pairf = nullptr;  // [N][mmax][3]  dE_k/dr_kj
+    double* e_s = nullptr;    // [N]
+    double* v_s = nullptr;    // [N]
+    // ---- chunk-sized intermediates (rows of the current chunk)
+    double* A = nullptr;     // [chunk][NvL2]
+    double* Bh = nullptr;    // [chunk][Pld]
+    double* W = nullptr;     // [chunk][Pld]
+    double* nrm = nullptr;   // [chunk]
+    double* part = nullptr;  // [2][max_ntn][chunk]  partial row-dots of the energy / variance tiles
+};
+
+// One quadratic-form group: rows whose atoms share the matrix (and, in sparse mode, the component set).
+struct GroupDesc {
+    int P = 0;            // descriptor components of this group (all of them in dense mode)
+    int K = 0;            // P padded to a multiple of 16 = reduction length and row length used
+    int nb = 0;           // n8-blocks per tile (tile width 8*nb)
+    int ntn = 0;          // tiles along N per matrix
+    const double* beta = nullptr;   // device [ntn*8*nb][K] padded, symmetric
+    const double* sigma = nullptr;  // same or nullptr
+    const int* table = nullptr;     // device [P]: component p -> nu1 | nu2<<8 | l<<16
+};
+
+// What the per-atom kernels need to know about a group (device array indexed by group id).
+struct GroupDev {
+    int P;
+    int K;
+    int ntn;
+    int pad_;
+    const int* table;
+};
+
+// stage entry points (each enqueues kernels through the Launcher)
+void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
+                     const int* types, int mmax, int sparse, int n_groups);
+
+// Descriptor rows [row0,row0+nrows): A -> ws.A, B^ -> bh_out (row r at (r - row0)*ld unless out_map given),
+// ||B|| -> nrm_out.  out_map (optional): row of atom k in bh_out/nrm_out is out_map[k] (used by the test hook).
+void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
+                     const GroupDev* groups, int row0, int nrows, double* bh_out, int ld, double* nrm_out,
+                     const int* out_map, bool write_A);
+
+void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_groups, int row0, int nrows, int ld,
+               int chunk_cap, bool want_variance, int sm_count);
+
+void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
+                  const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
+                  bool want_variance);
+
+void run_gather(Launcher& L, const Workspace& ws, int n, int mmax, double* e_out, double* f_out, double* var_out);
+
+void run_kick_drift(Launcher& L, const Grid& g, int n, double* x, double* v, const double* f, const int* types,
+                    const double* accel_half_dt /*[S] device: 0.5 dt kappa / m*/, double dt);
+void run_kick(Launcher& L, int n, double* v, const double* f, const int* types, const double* accel_half_dt);
+
+double measure_dmma_peak(int device);
+
+}  // namespace flare

@@ -1,0 +1,364 @@
+// neighbor.cu -- step a1: cell-list neighbour build ("all the neighbor atoms within a cutoff
+// radius"; R5-R7).  Produces, in cell-sorted atom order, a FULL (symmetric) neighbour
+// table nbr_idx[N][mmax] + nbr_cnt[N], the reverse-pair index rev[N][mmax] used by the atomics-free
+// force gather, the neighbour-species bitmask, and the grouping of atoms into quadratic-form rows.
+#include "kernels.cuh"
+
+namespace flare {
+
+// ------------------------------------------------------------------ wrap + cell assignment
+__global__ void k_cell_assign(Grid g, int n, const double* __restrict__ pos, int* __restrict__ cell_of,
+                              int* __restrict__ rank_in_cell, int* __restrict__ cell_cnt, int* __restrict__ flags) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double p[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+    int c = 0;
+    bool bad = false;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        if (!isfinite(p[d])) { bad = true; p[d] = 0.0; }
+        double w = g.pbc[d] ? wrap_coord(p[d], g.L[d]) : p[d];
+        int k = (int)floor(w * g.inv_cw[d]);
+        k = max(0, min(g.nc[d] - 1, k));
+        c += k * g.stride[d];
+    }
+    if (bad) atomicOr(flags, kFlagNonFinite);
+    cell_of[i] = c;
+    rank_in_cell[i] = atomicAdd(&cell_cnt[c], 1);
+}
+
+// ------------------------------------------------------------------ exclusive scan (3 launches)
+constexpr int kScanBlock = 1024;
+
+__global__ void k_scan_partial(int n, const int* __restrict__ in, int* __restrict__ out, int* __restrict__ block_sum) {
+    __shared__ int warp_tot[32];
+    int i = blockIdx.x * kScanBlock + threadIdx.x;
+    int v = (i < n) ? in[i] : 0;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(kFull, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_tot[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        int t = warp_tot[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(kFull, t, o);
+            if (lane >= o) t += y;
+        }
+        warp_tot[lane] = t;
+    }
+    __syncthreads();
+    int prefix = (w > 0 ? warp_tot[w - 1] : 0) + x - v;  // exclusive within the block
+    if (i < n) out[i] = prefix;
+    if (threadIdx.x == kScanBlock - 1) block_sum[blockIdx.x] = prefix + v;
+}
+
+// single block: exclusive scan of the block sums in place
+__global__ void k_scan_sums(int nb, int* __restrict__ block_sum) {
+    __shared__ int carry_s;
+    __shared__ int warp_tot[32];
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int base = 0; base < nb; base += kScanBlock) {
+        int i = base + threadIdx.x;
+        int v = (i < nb) ? block_sum[i] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(kFull, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[w] = x;
+        __syncthreads();
+        if (w == 0) {
+            int t = warp_tot[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(kFull, t, o);
+                if (lane >= o) t += y;
+            }
+            warp_tot[lane] = t;
+        }
+        __syncthreads();
+        int carry = carry_s;
+        int prefix = carry + (w > 0 ? warp_tot[w - 1] : 0) + x - v;
+        if (i < nb) block_sum[i] = prefix;
+        __syncthreads();
+        if (threadIdx.x == kScanBlock - 1) carry_s = prefix + v;
+        __syncthreads();
+    }
+}
+
+__global__ void k_scan_add(int n, int* __restrict__ out, const int* __restrict__ block_sum) {
+    int i = blockIdx.x * kScanBlock + threadIdx.x;
+    if (i < n) out[i] += block_sum[blockIdx.x];
+}
+
+// out[n] = out[n-1] + in[n-1]
+__global__ void k_scan_total(int n, const int* __restrict__ in, int* __restrict__ out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) out[n] = (n > 0) ? out[n - 1] + in[n - 1] : 0;
+}
+
+void exclusive_scan(Launcher& L, int n, const int* in, int* out /*[n+1]*/, int* block_sum) {
+    int nb = (n + kScanBlock - 1) / kScanBlock;
+    if (n > 0) {
+        L.launch(k_scan_partial, dim3(nb), dim3(kScanBlock), 0, n, in, out, block_sum);
+        L.launch(k_scan_sums, dim3(1), dim3(kScanBlock), 0, nb, block_sum);
+        L.launch(k_scan_add, dim3(nb), dim3(kScanBlock), 0, n, out, (const int*)block_sum);
+    }
+    L.launch(k_scan_total, dim3(1), dim3(32), 0, n, in, out);
+}
+
+// ------------------------------------------------------------------ counting sort by cell
+__global__ void k_scatter(int n, const int* __restrict__ cell_of, const int* __restrict__ rank_in_cell,
+                          const int* __restrict__ cell_start, int* __restrict__ order) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    order[cell_start[cell_of[i]] + rank_in_cell[i]] = i;
+}
+
+// The arrival order of atomicAdd inside a cell is not reproducible: sort each cell's (few) atoms by
+// their index in the caller's order so that the whole pipeline is run-to-run deterministic.
+__global__ void k_sort_cells(int n_cells, const int* __restrict__ cell_start, int* __restrict__ order) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cells) return;
+    int s = cell_start[c], e = cell_start[c + 1];
+    for (int a = s + 1; a < e; a++) {
+        int v = order[a];
+        int b = a - 1;
+        while (b >= s && order[b] > v) { order[b + 1] = order[b]; b--; }
+        order[b + 1] = v;
+    }
+}
+
+__global__ void k_gather_atoms(Grid g, int n, const double* __restrict__ pos, const int* __restrict__ types,
+                               const int* __restrict__ order, AtomS* __restrict__ atoms) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    int i = order[k];
+    AtomS a;
+    double p[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        if (!isfinite(p[d])) p[d] = 0.0;
+        if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
+    }
+    a.x = p[0]; a.y = p[1]; a.z = p[2];
+    a.type = types[i];
+    a.orig = i;
+    atoms[k] = a;
+}
+
+// ------------------------------------------------------------------ neighbour build: warp per atom
+__device__ __forceinline__ int fast_ranges(const Grid& g, int cf, int lo_out[2], int hi_out[2]) {
+    const int f = g.fast;
+    const int nc = g.nc[f];
+    if (g.pbc[f]) {
+        if (nc <= 3) { lo_out[0] = 0; hi_out[0] = nc - 1; return 1; }  // the whole column, each cell once
+        const int lo = cf - 1, hi = cf + 1;
+        if (lo < 0) { lo_out[0] = 0; hi_out[0] = hi; lo_out[1] = nc - 1; hi_out[1] = nc - 1; return 2; }
+        if (hi >= nc) { lo_out[0] = 0; hi_out[0] = 0; lo_out[1] = lo; hi_out[1] = nc - 1; return 2; }
+        lo_out[0] = lo; hi_out[0] = hi;
+        return 1;
+    }
+    lo_out[0] = max(cf - 1, 0);
+    hi_out[0] = min(cf + 1, nc - 1);
+    return 1;
+}
+
+// offsets of a slow dimension: returns count and the (wrapped) cell coordinates
+__device__ __forceinline__ int slow_cells(const Grid& g, int d, int c, int out[3]) {
+    const int nc = g.nc[d];
+    if (g.pbc[d]) {
+        if (nc == 1) { out[0] = 0; return 1; }
+        if (nc == 2) { out[0] = 0; out[1] = 1; return 2; }
+        out[0] = (c + nc - 1) % nc; out[1] = c; out[2] = (c + 1) % nc;
+        return 3;
+    }
+    int k = 0;
+    if (c - 1 >= 0) out[k++] = c - 1;
+    out[k++] = c;
+    if (c + 1 < nc) out[k++] = c + 1;
+    return k;
+}
+
+constexpr int kNbrWarps = 8;
+
+__global__ void __launch_bounds__(kNbrWarps * 32)
+k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int* __restrict__ cell_start, int mmax,
+            int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx, unsigned char* __restrict__ nmask,
+            int* __restrict__ flags) {
+    const int lane = threadIdx.x & 31;
+    const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
+    if (k >= n) return;
+    const AtomS me = load_atom(atoms + k);
+    int c[3];
+    c[0] = max(0, min(g.nc[0] - 1, (int)floor(me.x * g.inv_cw[0])));
+    c[1] = max(0, min(g.nc[1] - 1, (int)floor(me.y * g.inv_cw[1])));
+    c[2] = max(0, min(g.nc[2] - 1, (int)floor(me.z * g.inv_cw[2])));
+    int ca[3], cb[3], flo[2], fhi[2];
+    const int na = slow_cells(g, g.slow0, c[g.slow0], ca);
+    const int nb = slow_cells(g, g.slow1, c[g.slow1], cb);
+    const int nf = fast_ranges(g, c[g.fast], flo, fhi);
+    int* row = nbr_idx + (size_t)k * mmax;
+    int cnt = 0;
+    unsigned mask = 0;
+    const double* rc2 = bs.rc2 + me.type * bs.S;
+    for (int ib = 0; ib < nb; ib++)
+        for (int ia = 0; ia < na; ia++) {
+            const int base = ca[ia] * g.stride[g.slow0] + cb[ib] * g.stride[g.slow1];
+            for (int r = 0; r < nf; r++) {
+                const int s = cell_start[base + flo[r]];
+                const int e = cell_start[base + fhi[r] + 1];
+                for (int q0 = s; q0 < e; q0 += 32) {
+                    const int q = q0 + lane;
+                    bool hit = false;
+                    int tj = 0;
+                    if (q < e && q != k) {
+                        const AtomS o = load_atom(atoms + q);
+                        double dx, dy, dz;
+                        displacement(g, me, o, dx, dy, dz);
+                        tj = o.type;
+                        hit = dist2_canonical(dx, dy, dz) < rc2[tj];  // strict (R6)
+                    }
+                    const unsigned b = __ballot_sync(kFull, hit);
+                    if (hit) {
+                        const int slot = cnt + __popc(b & ((1u << lane) - 1u));
+                        if (slot < mmax) row[slot] = q;
+                        mask |= 1u << tj;
+                    }
+                    cnt += __popc(b);
+                }
+            }
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mask |= __shfl_xor_sync(kFull, mask, o);
+    if (lane == 0) {
+        if (cnt > mmax) { atomicOr(flags, kFlagNeighborOverflow); cnt = mmax; }
+        nbr_cnt[k] = cnt;
+        nmask[k] = (unsigned char)mask;
+    }
+}
+
+// rev[k][s] = slot of k in the row of j = nbr_idx[k][s]  (exists because cutoffs are symmetric, R5)
+__global__ void __launch_bounds__(kNbrWarps * 32)
+k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx,
+                unsigned char* __restrict__ rev) {
+    const int lane = threadIdx.x & 31;
+    const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
+    if (k >= n) return;
+    const int cnt = nbr_cnt[k];
+    for (int s = 0; s < cnt; s++) {
+        const int j = nbr_idx[(size_t)k * mmax + s];
+        const int cj = nbr_cnt[j];
+        int found = 0;
+        for (int b = 0; b < cj; b += 32) {
+            const int t = b + lane;
+            const bool eq = (t < cj) && (nbr_idx[(size_t)j * mmax + t] == k);
+            const unsigned m = __ballot_sync(kFull, eq);
+            if (m) { found = b + __ffs(m) - 1; break; }
+        }
+        if (lane == 0) rev[(size_t)k * mmax + s] = (unsigned char)found;
+    }
+}
+
+// ------------------------------------------------------------------ grouping into quadratic-form rows
+// Group of an atom: dense mode -> its species; sparse mode -> (species, neighbour-species mask).
+__device__ __forceinline__ int group_of(int type, unsigned mask, int S, int sparse) {
+    return sparse ? type * (1 << S) + (int)mask : type;
+}
+
+constexpr int kGroupBlock = 1024;
+
+__global__ void __launch_bounds__(kGroupBlock)
+k_group_hist(int n, int S, int sparse, int n_groups, const AtomS* __restrict__ atoms,
+             const unsigned char* __restrict__ nmask, int* __restrict__ hist /*[n_blocks][n_groups]*/) {
+    __shared__ int h[kMaxGroups];
+    for (int t = threadIdx.x; t < n_groups; t += blockDim.x) h[t] = 0;
+    __syncthreads();
+    int k = blockIdx.x * kGroupBlock + threadIdx.x;
+    if (k < n) atomicAdd(&h[group_of(atoms[k].type, nmask[k], S, sparse)], 1);
+    __syncthreads();
+    for (int t = threadIdx.x; t < n_groups; t += blockDim.x) hist[(size_t)blockIdx.x * n_groups + t] = h[t];
+}
+
+// one thread per group walks the blocks; then thread 0 lays the groups out one after another
+__global__ void k_group_scan(int n_blocks, int n_groups, int* __restrict__ hist, int* __restrict__ group_start) {
+    __shared__ int tot[kMaxGroups + 1];
+    int gidx = threadIdx.x;
+    if (gidx < n_groups) {
+        int run = 0;
+        for (int b = 0; b < n_blocks; b++) {
+            int v = hist[(size_t)b * n_groups + gidx];
+            hist[(size_t)b * n_groups + gidx] = run;
+            run += v;
+        }
+        tot[gidx] = run;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int run = 0;
+        for (int t = 0; t < n_groups; t++) { group_start[t] = run; run += tot[t]; }
+        group_start[n_groups] = run;
+    }
+}
+
+__global__ void __launch_bounds__(kGroupBlock)
+k_group_assign(int n, int S, int sparse, int n_groups, const AtomS* __restrict__ atoms,
+               const unsigned char* __restrict__ nmask, const int* __restrict__ hist,
+               const int* __restrict__ group_start, int* __restrict__ row_of, int* __restrict__ atom_of_row,
+               unsigned char* __restrict__ gid_out) {
+    __shared__ int wcnt[32][kMaxGroups];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int t = threadIdx.x; t < 32 * kMaxGroups; t += blockDim.x) (&wcnt[0][0])[t] = 0;
+    __syncthreads();
+    const int k = blockIdx.x * kGroupBlock + threadIdx.x;
+    const int gid = (k < n) ? group_of(atoms[k].type, nmask[k], S, sparse) : -1;
+    const unsigned peers = __match_any_sync(kFull, gid);
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    if (gid >= 0 && rank == 0) wcnt[w][gid] = __popc(peers);
+    __syncthreads();
+    if (gid >= 0) {
+        int before = 0;
+        for (int ww = 0; ww < w; ww++) before += wcnt[ww][gid];
+        const int row = group_start[gid] + hist[(size_t)blockIdx.x * n_groups + gid] + before + rank;
+        row_of[k] = row;
+        atom_of_row[row] = k;
+        gid_out[k] = (unsigned char)gid;
+    }
+}
+
+// ------------------------------------------------------------------ host-side driver of a1
+void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
+                     const int* types, int mmax, int sparse, int n_groups) {
+    if (n == 0) return;
+    const int tb = 256;
+    L.memset(ws.cell_cnt, 0, sizeof(int) * (size_t)g.n_cells);
+    L.launch(k_cell_assign, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, ws.cell_of, ws.rank_in_cell, ws.cell_cnt,
+             ws.flags);
+    exclusive_scan(L, g.n_cells, ws.cell_cnt, ws.cell_start, ws.scan_tmp);
+    L.launch(k_scatter, dim3((n + tb - 1) / tb), dim3(tb), 0, n, (const int*)ws.cell_of, (const int*)ws.rank_in_cell,
+             (const int*)ws.cell_start, ws.order);
+    L.launch(k_sort_cells, dim3((g.n_cells + tb - 1) / tb), dim3(tb), 0, g.n_cells, (const int*)ws.cell_start, ws.order);
+    L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order, ws.atoms);
+    const int nwb = (n + kNbrWarps - 1) / kNbrWarps;
+    L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bs, n, (const AtomS*)ws.atoms,
+             (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+    L.launch(k_reverse_index, dim3(nwb), dim3(kNbrWarps * 32), 0, n, mmax, (const int*)ws.nbr_cnt,
+             (const int*)ws.nbr_idx, ws.rev);
+    const int ngb = (n + kGroupBlock - 1) / kGroupBlock;
+    L.launch(k_group_hist, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
+             (const unsigned char*)ws.nmask, ws.group_hist);
+    L.launch(k_group_scan, dim3(1), dim3(kMaxGroups), 0, ngb, n_groups, ws.group_hist, ws.group_start);
+    L.launch(k_group_assign, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
+             (const unsigned char*)ws.nmask, (const int*)ws.group_hist, (const int*)ws.group_start, ws.row_of,
+             ws.atom_of_row, ws.gid);
+}
+
+}  // namespace flare

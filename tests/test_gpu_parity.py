@@ -1,0 +1,282 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars (BASELINE.json north_star): neighbour sets bit-exact; energies, variances
+within 1e-10 relative; forces within 1e-12 eV/A absolute + 1e-10 relative.
+"""
+import numpy as np
+import pytest
+
+from paper_2204_12573_b200 import workloads as w
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-10
+ATOL_F = 1e-12  # eV/A
+ATOL_E = 1e-12  # eV, guards E ~ 0 (isolated atoms)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    return torch
+
+
+@pytest.fixture(scope="module")
+def flare():
+    from paper_2204_12573_b200 import flare as fl
+
+    fl.load_library()
+    return fl
+
+
+def dev(torch, a, dtype):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device="cuda")
+
+
+def gpu_compute(torch, flare, s, variance=True, **kw):
+    ctx = flare.from_system(s, variance=variance, **kw)
+    ctx.bind(s.n_atoms)
+    e, f, v = ctx.compute(dev(torch, s.pos, torch.float64), dev(torch, s.types, torch.int32), s.box, s.pbc,
+                          variances=variance)
+    torch.cuda.synchronize()
+    return ctx, e.cpu().numpy(), f.cpu().numpy(), (v.cpu().numpy() if v is not None else None)
+
+
+def assert_close(got, want, atol, what):
+    err = np.abs(got - want)
+    tol = atol + RTOL * np.abs(want)
+    bad = err > tol
+    assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} outside tolerance; worst err {err.max():.3e} " \
+                          f"(|want| max {np.abs(want).max():.3e})"
+
+
+def assert_parity(oracle, torch, flare, s, variance=True, nbr_method=1, **kw):
+    ctx, e, f, v = gpu_compute(torch, flare, s, variance, **kw)
+    E, F, V = oracle.compute(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta,
+                             s.sigma if variance else None, nbr_method=nbr_method)
+    # neighbour sets: bit-exact
+    cnt_o, idx_o = oracle.neighbors(s.pos, s.types, s.box, s.pbc, s.r_cut, nbr_method, cap=ctx.get_option(1))
+    cnt_g, idx_g = ctx.neighbors()
+    assert np.array_equal(cnt_g, cnt_o)
+    assert np.array_equal(idx_g, idx_o)
+    assert_close(e, E, ATOL_E, "E")
+    assert_close(f, F, ATOL_F, "F")
+    if variance:
+        assert_close(v, V, 1e-15, "V")
+    return ctx, (e, f, v), (E, F, V)
+
+
+# ----------------------------------------------------------------------------- BASELINE configs 1 and 2 in full
+
+
+def test_config1_full(oracle, torch, flare):
+    s = w.config1()
+    ctx, got, want = assert_parity(oracle, torch, flare, s, nbr_method=0)
+    assert np.abs(got[1].sum(0)).max() < 1e-11  # zero net force
+    # descriptors at the a3 boundary
+    bh, nrm = ctx.descriptors()
+    for i in (0, 100, 255):
+        _, _, Bh, n0 = oracle.descriptor(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, i)
+        np.testing.assert_allclose(bh[i], Bh, atol=1e-13)
+        assert abs(nrm[i] - n0) < 1e-12 * n0
+
+
+def test_config2_full(oracle, torch, flare):
+    s = w.config2()
+    ctx, got, want = assert_parity(oracle, torch, flare, s, nbr_method=0)
+    bh, nrm = ctx.descriptors()
+    for i in (0, 500, 863, 864, 1263):  # Pt bulk, Pt surface, H
+        _, _, Bh, n0 = oracle.descriptor(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, i)
+        np.testing.assert_allclose(bh[i], Bh, atol=1e-13)
+    assert np.abs(got[1].sum(0)).max() < 1e-10
+
+
+# ----------------------------------------------------------------------------- basis sizes, several tiles + ragged tails
+
+
+@pytest.mark.parametrize("n_max,l_max", [(1, 0), (3, 1), (4, 2), (7, 3), (3, 4), (2, 5), (2, 6), (5, 6)])
+def test_basis_sizes_on_a_small_tile(oracle, torch, flare, n_max, l_max):
+    s = w.tile_like_c3(6, 3, n_max=n_max, l_max=l_max)  # 216 Pt + 18 H
+    assert_parity(oracle, torch, flare, s)
+
+
+def test_paper_basis_7_3_dimension_420(oracle, torch, flare):
+    """The paper's own model size: 2 species, n_max 7, l_max 3 -> 420."""
+    s = w.tile_like_c3(8, 4, n_max=7, l_max=3)
+    assert s.P == 420
+    assert_parity(oracle, torch, flare, s)
+
+
+@pytest.mark.parametrize("chunk", [64, 100, 1000])
+def test_chunking_is_exact(oracle, torch, flare, chunk):
+    """Step a8: chunked intermediates must not change any result; 100 gives ragged tails."""
+    s = w.tile_like_c3(8, 4, n_max=4, l_max=3)
+    ctx0, e0, f0, v0 = gpu_compute(torch, flare, s)
+    ctx1, e1, f1, v1 = gpu_compute(torch, flare, s, chunk_atoms=chunk)
+    assert ctx1.get_option(2) == min(chunk, s.n_atoms)
+    assert np.array_equal(e0, e1) and np.array_equal(f0, f1) and np.array_equal(v0, v1)
+    assert_parity(oracle, torch, flare, s, chunk_atoms=chunk)
+
+
+def test_run_to_run_determinism(torch, flare):
+    s = w.config2()
+    _, e0, f0, v0 = gpu_compute(torch, flare, s)
+    _, e1, f1, v1 = gpu_compute(torch, flare, s)
+    assert np.array_equal(e0, e1) and np.array_equal(f0, f1) and np.array_equal(v0, v1)
+
+
+def test_variance_off_matches_variance_on(torch, flare):
+    s = w.config2()
+    _, e0, f0, _ = gpu_compute(torch, flare, s, variance=False)
+    _, e1, f1, _ = gpu_compute(torch, flare, s, variance=True)
+    assert np.array_equal(e0, e1) and np.array_equal(f0, f1)
+
+
+# ----------------------------------------------------------------------------- edge and degenerate cases
+
+
+def _mk(pos, types, box, pbc, S, n_max=3, l_max=2, seed=0):
+    rng = np.random.default_rng(seed)
+    P = w.num_descriptors(S, n_max, l_max)
+    r_cut = w.R_CUT_1 if S == 1 else w.R_CUT_2
+    mass = np.array([w.MASS_PT, w.MASS_H])[:S]
+    s = w.System("edge", np.asarray(pos, float).reshape(-1, 3), np.asarray(types, np.int32), np.asarray(box, float),
+                 np.asarray(pbc, np.int32), mass, r_cut, n_max, l_max)
+    s.beta = w.random_beta(rng, S, P)
+    s.sigma = w.random_sigma(rng, S, P)
+    return s
+
+
+def test_empty_and_single_atom(oracle, torch, flare):
+    box = np.diag([30.0, 30, 30]).reshape(9)
+    s = _mk(np.zeros((0, 3)), [], box, [1, 1, 1], 1)
+    ctx, e, f, v = gpu_compute(torch, flare, s)
+    assert e.size == 0 and f.size == 0
+    s = _mk([[1.0, 2, 3]], [0], box, [1, 1, 1], 1)
+    ctx, e, f, v = gpu_compute(torch, flare, s)
+    assert e[0] == 0 and v[0] == 0 and np.all(f == 0)  # R8: empty neighbourhood
+    # a dimer plus an isolated atom
+    s = _mk([[1.0, 2, 3], [20, 20, 20], [21.1, 20.2, 19.7]], [0, 1, 0], box, [1, 1, 1], 2)
+    assert_parity(oracle, torch, flare, s, nbr_method=0)
+
+
+def test_open_and_mixed_boundaries_and_unwrapped_input(oracle, torch, flare):
+    rng = np.random.default_rng(11)
+    n = 300
+    pos = rng.uniform(0, 22, (n, 3))
+    keep = [0]
+    for i in range(1, n):
+        if np.min(np.linalg.norm(pos[keep] - pos[i], axis=1)) > 1.1:
+            keep.append(i)
+    pos = pos[keep]
+    types = rng.integers(0, 2, len(keep))
+    box = np.diag([22.0, 22, 22]).reshape(9)
+    for pbc in ([0, 0, 0], [1, 0, 1], [1, 1, 1]):
+        shifted = pos.copy()
+        for d in range(3):
+            if pbc[d]:
+                shifted[:, d] += 22.0 * rng.integers(-3, 4, len(keep))  # any periodic image (R6)
+            else:
+                shifted[:, d] += -5.0  # atoms outside [0,L) in an open dimension are legal
+        s = _mk(shifted, types, box, pbc, 2, n_max=3, l_max=3, seed=12)
+        assert_parity(oracle, torch, flare, s, nbr_method=0)
+
+
+def test_fewer_than_three_cells_per_dimension(oracle, torch, flare):
+    """Box lengths between 2 and 3 cutoffs: the 27-cell stencil would revisit cells (R7)."""
+    rng = np.random.default_rng(13)
+    pos, types, box, pbc = w.fcc_bulk(3, w.A_PT, 0.05, rng)  # L = 11.76 A: 2 cells of >= 4.25 per dimension
+    s = _mk(pos, types, box, pbc, 1, n_max=4, l_max=3, seed=14)
+    assert_parity(oracle, torch, flare, s, nbr_method=0)
+    pos, types, box, pbc = w.fcc_bulk(4, w.A_PT, 0.05, rng)  # L = 15.68: 3 cells
+    s = _mk(pos, types, box, pbc, 1, n_max=4, l_max=3, seed=15)
+    assert_parity(oracle, torch, flare, s, nbr_method=0)
+
+
+def test_perfect_lattice_zero_force(torch, flare):
+    pos, types, box, pbc = w.fcc_bulk(4, w.A_PT, 0.0, None)
+    s = _mk(pos, types, box, pbc, 1, n_max=6, l_max=3, seed=16)
+    _, e, f, v = gpu_compute(torch, flare, s)
+    assert np.abs(f).max() < 1e-12 and np.ptp(e) < 1e-13
+
+
+def test_error_codes(torch, flare):
+    box = np.diag([30.0, 30, 30]).reshape(9)
+    s = _mk(np.random.default_rng(1).uniform(0, 30, (50, 3)), np.zeros(50), box, [1, 1, 1], 1)
+    ctx = flare.from_system(s)
+    pos, types = dev(torch, s.pos, torch.float64), dev(torch, s.types, torch.int32)
+    with pytest.raises(flare.FlareError) as ei:  # not bound
+        ctx.n_atoms = 50
+        ctx.compute(pos, types, s.box, s.pbc)
+    assert ei.value.code == -9
+    ctx.bind(50)
+    with pytest.raises(flare.FlareError) as ei:  # periodic box < 2 r_cut
+        ctx.compute(pos, types, np.diag([8.0, 30, 30]).reshape(9), [1, 1, 1])
+    assert ei.value.code == -2
+    tri = np.diag([30.0, 30, 30])
+    tri[1, 0] = 2.0
+    with pytest.raises(flare.FlareError) as ei:  # triclinic
+        ctx.compute(pos, types, tri.reshape(9), [1, 1, 1])
+    assert ei.value.code == -3
+    with pytest.raises(flare.FlareError) as ei:  # variance without sigma
+        c2 = flare.from_system(s, variance=False).bind(50)
+        c2.compute(pos, types, s.box, s.pbc, variances=True)
+    assert ei.value.code == -1
+    bad = s.pos.copy()
+    bad[7, 1] = np.nan
+    with pytest.raises(flare.FlareError) as ei:
+        ctx.compute(dev(torch, bad, torch.float64), types, s.box, s.pbc)
+    assert ei.value.code == -7
+    # neighbour overflow: 40 atoms in a 2 A ball with room for 8 neighbours
+    rng = np.random.default_rng(2)
+    s2 = _mk(15 + rng.uniform(-1, 1, (40, 3)), np.zeros(40), box, [1, 1, 1], 1)
+    c3 = flare.from_system(s2, max_neighbors=8).bind(40)
+    with pytest.raises(flare.FlareError) as ei:
+        c3.compute(dev(torch, s2.pos, torch.float64), dev(torch, s2.types, torch.int32), s2.box, s2.pbc)
+    assert ei.value.code == -5
+    with pytest.raises(flare.FlareError) as ei:  # asymmetric r_cut (R5)
+        flare.Flare([1.0, 1.0], 2, 1, [[3.0, 2.0], [2.5, 3.0]], np.zeros((2, 20, 20)))
+    assert ei.value.code == -1
+    with pytest.raises(flare.FlareError) as ei:  # l_max out of the compiled range
+        flare.Flare([1.0], 2, 7, [[3.0]], np.zeros((1, 24, 24)))
+    assert ei.value.code == -8
+
+
+def test_many_neighbours_more_than_a_warp(oracle, torch, flare):
+    """Dense blob: up to ~60 neighbours per atom exercises the >32-neighbour loops."""
+    rng = np.random.default_rng(21)
+    pos = rng.uniform(0, 9.0, (400, 3))
+    keep = [0]
+    for i in range(1, len(pos)):
+        if np.min(np.linalg.norm(pos[keep] - pos[i], axis=1)) > 1.25:
+            keep.append(i)
+    pos = pos[keep] + 10.0
+    s = _mk(pos, np.zeros(len(keep)), np.diag([30.0, 30, 30]).reshape(9), [1, 1, 1], 1, n_max=3, l_max=2, seed=22)
+    cnt, _ = oracle.neighbors(s.pos, s.types, s.box, s.pbc, s.r_cut, 0, cap=255)
+    assert cnt.max() > 40
+    assert_parity(oracle, torch, flare, s, nbr_method=0, max_neighbors=int(cnt.max()) + 1)
+
+
+def test_host_entry_point_matches_device_entry_point(torch, flare):
+    s = w.config2()
+    ctx, e, f, v = gpu_compute(torch, flare, s)
+    eh, fh, vh = ctx.compute_host(s.pos, s.types, s.box, s.pbc, variances=True)
+    assert np.array_equal(e, eh) and np.array_equal(f, fh) and np.array_equal(v, vh)
+
+
+# ----------------------------------------------------------------------------- larger systems: sampled parity
+
+
+def test_tile_16k_atoms_sampled(oracle, torch, flare):
+    s = w.tile_like_c3(48, 24)  # 13 824 Pt + 1152 H, P = 544
+    ctx, e, f, v = gpu_compute(torch, flare, s)
+    rng = np.random.default_rng(31)
+    sel = np.concatenate([rng.choice(13824, 24, replace=False), 13824 + rng.choice(1152, 8, replace=False)])
+    E, F, V = oracle.compute_selected(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, sel)
+    assert_close(e[sel], E, ATOL_E, "E")
+    assert_close(f[sel], F, ATOL_F, "F")
+    assert_close(v[sel], V, 1e-15, "V")
+    cnt_o, idx_o = oracle.neighbors(s.pos, s.types, s.box, s.pbc, s.r_cut, 1, cap=ctx.get_option(1))
+    cnt_g, idx_g = ctx.neighbors()
+    assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+    assert np.abs(f.sum(0)).max() < 1e-9
