@@ -141,6 +141,14 @@ int flare_set_state_host(flare_ctx* ctx, const double* pos, const double* vel, c
                          const double box[9], const int pbc[3]);
 
 /*
+ * Optional: supply the forces (eV/A, [N][3]) that belong to the state just set -- e.g. when resuming
+ * from a checkpoint -- so that flare_step does not re-evaluate them before its first half-kick.
+ * The caller vouches that they are the forces of those positions.  Device / host pointer versions.
+ */
+int flare_set_forces(flare_ctx* ctx, const double* f);
+int flare_set_forces_host(flare_ctx* ctx, const double* f);
+
+/*
  * n_steps of velocity Verlet (R12): v += dt/2 KAPPA F/m; x += dt v; wrap; F = F(x); v += dt/2 KAPPA F/m.
  * The neighbour list is rebuilt every step.  Forces of the current positions are evaluated
  * first if they are not yet valid.  want_variance != 0 also evaluates V_i each step.  Asynchronous.

@@ -549,6 +549,21 @@ int flare_set_state_host(flare_ctx* c, const double* pos, const double* vel, con
     return set_state_impl(c, pos, vel, types, box, pbc, cudaMemcpyHostToDevice);
 }
 
+static int set_forces_impl(flare_ctx* c, const double* f, cudaMemcpyKind kind) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->state_set) return fail(c, FLARE_ERR_NOT_BOUND, "flare_set_state has not been called");
+    if (!f && c->n > 0) return fail(c, FLARE_ERR_INVALID_ARG, "forces pointer is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    if (c->n > 0 && f != c->ws.f)
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.f, f, sizeof(double) * 3 * (size_t)c->n, kind, c->stream));
+    c->forces_valid = true;
+    return FLARE_OK;
+}
+
+int flare_set_forces(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyDeviceToDevice); }
+int flare_set_forces_host(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyHostToDevice); }
+
 int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
     int rc = need_bound(c);
     if (rc) return rc;
@@ -559,7 +574,7 @@ int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
     const int n = (int)c->n;
     Workspace& w = c->ws;
     double* var = want_variance ? w.var : nullptr;
-    if (!c->forces_valid || (want_variance && !c->var_valid)) {
+    if (!c->forces_valid || (want_variance && !c->var_valid && n_steps == 0)) {
         rc = evaluate(c, w.x, w.types, w.e, w.f, var);
         if (rc) return rc;
         c->forces_valid = true;

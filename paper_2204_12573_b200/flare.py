@@ -28,7 +28,7 @@ PHASES = ("neighbor", "descriptor", "qform", "backprop", "gather", "integrate")
 EXPORTS = (
     "flare_create", "flare_destroy", "flare_num_descriptors", "flare_set_option", "flare_get_option",
     "flare_workspace_bytes", "flare_bind", "flare_compute", "flare_compute_host", "flare_check",
-    "flare_set_state", "flare_set_state_host", "flare_step", "flare_get_state", "flare_get_state_host",
+    "flare_set_state", "flare_set_state_host", "flare_set_forces", "flare_set_forces_host", "flare_step", "flare_get_state", "flare_get_state_host",
     "flare_get_neighbors", "flare_get_descriptors", "flare_get_timings", "flare_kernel_launches",
     "flare_measure_fp64_dmma_peak", "flare_last_error",
 )
@@ -67,6 +67,8 @@ def load_library():
     lib.flare_check.argtypes = [vp]
     lib.flare_set_state.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.flare_set_state_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.flare_set_forces.argtypes = [vp, vp]
+    lib.flare_set_forces_host.argtypes = [vp, vp]
     lib.flare_step.argtypes = [vp, dbl, i32, i32]
     lib.flare_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.flare_get_state_host.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -241,6 +243,15 @@ class Flare:
             pv = None if vel is None else self._dev(vel, torch.float64, (n, 3))
             self._check(self._lib.flare_set_state(self._ctx, self._dev(pos, torch.float64, (n, 3)), pv,
                                                   self._dev(types, torch.int32, (n,)), _hp(boxh), _hp(pbch)))
+
+    def set_forces(self, f):
+        """Forces belonging to the state just set (skips the initial evaluation of step())."""
+        n = self.n_atoms
+        if isinstance(f, np.ndarray):
+            f = _np(f, np.float64).reshape(n, 3)
+            self._check(self._lib.flare_set_forces_host(self._ctx, _hp(f)))
+        else:
+            self._check(self._lib.flare_set_forces(self._ctx, self._dev(f, self._torch.float64, (n, 3))))
 
     def step(self, dt_fs: float, n_steps: int = 1, want_variance: bool = False):
         self._check(self._lib.flare_step(self._ctx, float(dt_fs), int(n_steps), 1 if want_variance else 0))

@@ -1,0 +1,123 @@
+"""GPU molecular dynamics (step a9) against the oracle: trajectories are chaotic, so parity is by
+RE-SYNC (feed the GPU's positions to the oracle and compare E, F, V there) plus short-run agreement,
+conserved-quantity traces and time reversal."""
+import numpy as np
+import pytest
+
+from paper_2204_12573_b200 import workloads as w
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    return torch
+
+
+@pytest.fixture(scope="module")
+def flare():
+    from paper_2204_12573_b200 import flare as fl
+
+    fl.load_library()
+    return fl
+
+
+def start(torch, flare, s, **kw):
+    ctx = flare.from_system(s, **kw).bind(s.n_atoms)
+    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)  # host arrays -> flare_set_state_host
+    return ctx
+
+
+def total_energy(st, s):
+    ke = w.kinetic_energy(st["vel"], s.types, s.mass)
+    return ke + st["E"].sum(), ke
+
+
+def test_config1_ten_steps_match_oracle_trajectory(oracle, torch, flare):
+    s = w.config1()
+    ctx = start(torch, flare, s)
+    ctx.step(1.0, 10, want_variance=True)
+    st = ctx.get_state_host(variances=True)
+    ref = oracle.step(s.pos, s.vel, s.types, s.mass, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, 1.0, 10)
+    # 10 steps: round-off has not been amplified yet
+    assert np.abs(st["pos"] - ref["pos"]).max() < 1e-10
+    assert np.abs(st["vel"] - ref["vel"]).max() < 1e-12
+    assert np.abs(st["F"] - ref["F"]).max() < 1e-9
+    assert np.abs(st["E"] - ref["E"]).max() < 1e-10
+    assert np.abs(st["V"] - ref["V"]).max() < 1e-13
+    h_gpu, _ = total_energy(st, s)
+    assert abs(h_gpu - (ref["pe"][-1] + ref["ke"][-1])) < 1e-9
+
+
+def test_config2_resync_parity_during_md(oracle, torch, flare):
+    s = w.config2()
+    ctx = start(torch, flare, s)
+    h = []
+    for block in range(4):
+        ctx.step(0.5, 25, want_variance=True)
+        st = ctx.get_state_host(variances=True)
+        E, F, V = oracle.compute(st["pos"], s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma)
+        assert np.all(np.abs(st["E"] - E) <= 1e-12 + 1e-10 * np.abs(E))
+        assert np.all(np.abs(st["F"] - F) <= 1e-12 + 1e-10 * np.abs(F))
+        assert np.all(np.abs(st["V"] - V) <= 1e-15 + 1e-10 * np.abs(V))
+        h.append(total_energy(st, s))
+    h0 = w.kinetic_energy(s.vel, s.types, s.mass)
+    drift = max(abs(x[0] - h[0][0]) for x in h)
+    assert drift < 2e-3 * h0, (drift, h0)  # NVE: conserved to a small fraction of the kinetic energy
+    # positions stay wrapped
+    L = np.asarray(s.box).reshape(3, 3).diagonal()
+    assert np.all(st["pos"] >= 0) and np.all(st["pos"] < L)
+
+
+def test_drift_scales_with_dt_squared_and_time_reversal(torch, flare):
+    s = w.config1()
+    fl = []
+    for dt, n in ((4.0, 20), (2.0, 40)):
+        ctx = start(torch, flare, s, variance=False)
+        ctx.step(dt, 0)
+        h0, _ = total_energy(ctx.get_state_host(), s)
+        worst = 0.0
+        for _ in range(n // 5):
+            ctx.step(dt, 5)
+            hh, _ = total_energy(ctx.get_state_host(), s)
+            worst = max(worst, abs(hh - h0))
+        fl.append(worst)
+    assert 2.0 < fl[0] / fl[1] < 8.0, fl
+    # time reversal
+    ctx = start(torch, flare, s, variance=False)
+    ctx.step(1.0, 20)
+    st = ctx.get_state_host()
+    ctx.set_state(st["pos"], -st["vel"], s.types, s.box, s.pbc)
+    ctx.step(1.0, 20)
+    back = ctx.get_state_host()
+    L = np.asarray(s.box).reshape(3, 3).diagonal()
+    d = back["pos"] - s.pos
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() < 1e-9
+    assert np.abs(-back["vel"] - s.vel).max() < 1e-11
+    # momentum conservation
+    m = s.mass[s.types][:, None]
+    assert np.abs((m * back["vel"]).sum(0) + (m * s.vel).sum(0)).max() < 1e-11
+
+
+def test_supplied_forces_skip_the_initial_evaluation(torch, flare):
+    s = w.config1()
+    ctx = start(torch, flare, s, variance=False)
+    ctx.step(1.0, 3)
+    a = ctx.get_state_host()
+    ctx2 = start(torch, flare, s, variance=False)
+    ctx2.step(1.0, 1)
+    mid = ctx2.get_state_host()
+    n0 = ctx2.kernel_launches()
+    ctx2.set_state(mid["pos"], mid["vel"], s.types, s.box, s.pbc)
+    ctx2.set_forces(mid["F"])
+    ctx2.step(1.0, 2)
+    per_eval = (ctx2.kernel_launches() - n0)
+    b = ctx2.get_state_host()
+    assert np.array_equal(a["pos"], b["pos"]) and np.array_equal(a["vel"], b["vel"])
+    ctx3 = start(torch, flare, s, variance=False)
+    n1 = ctx3.kernel_launches()
+    ctx3.step(1.0, 2)
+    assert ctx3.kernel_launches() - n1 > per_eval  # that one evaluated the initial forces as well
