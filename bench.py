@@ -279,7 +279,9 @@ def run_ours(args):
     roofline = {
         "bound": "tensor", "kernel": "k_qform (FP64 DMMA grouped GEMM, beta + Sigma forms)",
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
-        "traffic": None,
+        # dram__bytes_read+write of k_qform per atom row, from the ncu --set full capture in
+        # profiles/r01_qform_full.md (1.771 GB for the 205 184-row launch), scaled to one step's rows
+        "traffic": 8630.0 * n if P == 544 else None,
         "peak_source": "FP64 DMMA issue peak measured live by flare_measure_fp64_dmma_peak "
                        "(MEASURED_PEAKS.json has no FP64 entry; its sustained bf16 x nominal 45/2250 gives "
                        f"{derived:.1f} TFLOP/s)" if derived else "FP64 DMMA issue peak measured live",
