@@ -1,17 +1,29 @@
 // descriptor.cu -- steps a2 + a3: per-pair basis, A accumulation, B2 contraction, normalisation
-// (P:L123-129).  One warp per atom: neighbours are spread across lanes for the basis evaluation
-// (sqrt, sincospi, Chebyshev and Y_lm recurrences), their g~_n and Y_lm values are staged in shared
-// memory, then the lanes switch to owning (n,l,m) components and sum over the staged neighbours
-// -- no shuffle reduction over 256+ components is needed.  A stays in shared memory for the B2
-// contraction; B^ goes to the quadratic-form row of the atom.
+// (P:L123-129).  One warp per atom:
+//   1. neighbours are spread across lanes for the basis evaluation (sqrt, sincospi, Chebyshev and
+//      Y_lm recurrences); g~_n and Y_lm of up to 32 neighbours are staged in shared memory;
+//   2. A[nu,lm] = sum_j [s_j = s] g~_n(j) Y_lm(j) is a small dense contraction over the neighbours
+//      (an [N_nu x M] . [M x L^2] product); it runs on the FP64 tensor pipe (mma.sync m8n8k4) with
+//      the species selection folded into the A-operand, so no shuffle reduction over the 256+
+//      components and no per-component shared-memory loop is needed;
+//   3. B[nu1<=nu2, l] = sum_m A[nu1,l,m] A[nu2,l,m]: one (nu1,nu2) pair per lane, all l at once, so a
+//      warp writes 32 x (l_max+1) consecutive doubles of the B^ row (fully coalesced); two passes
+//      (norm, then scaled store) recompute the cheap contraction instead of holding B in registers.
 #include "kernels.cuh"
 
 namespace flare {
 
 constexpr int kDescWarps = 4;
 
-__host__ __device__ inline int desc_warp_doubles(int n_max, int L2, int NvL2) {
-    return 32 * (n_max | 1) + 32 * (L2 | 1) + NvL2 + 16;
+__host__ __device__ inline int desc_warp_doubles(int n_max, int L2, int Nv) {
+    // g[32][n_max|1], Y[32][L2|1], A[Nv][L2|1], species[32] (ints, 16 doubles)
+    return 32 * (n_max | 1) + 32 * (L2 | 1) + Nv * (L2 | 1) + 16;
+}
+
+__device__ __forceinline__ void dmma884_d(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
 }
 
 template <int LMAX>
@@ -21,23 +33,26 @@ k_descriptor(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const 
              const unsigned char* __restrict__ gid, const GroupDev* __restrict__ groups, int row0, int nrows,
              double* __restrict__ A_out, double* __restrict__ bh_out, int ld, double* __restrict__ nrm_out,
              const int* __restrict__ out_map) {
-    constexpr int L2 = (LMAX + 1) * (LMAX + 1);
-    constexpr int YS = L2 | 1;
+    constexpr int L = LMAX + 1;
+    constexpr int L2 = L * L;
+    constexpr int YS = L2 | 1;  // odd row strides: conflict-free column access across rows
+    constexpr int AS = L2 | 1;
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int local = blockIdx.x * kDescWarps + warp;
     if (local >= nrows) return;  // warps are independent: only __syncwarp below
+    const int g8 = lane >> 2, t4 = lane & 3;
     const int GS = bs.n_max | 1;
-    const int nL2 = bs.n_max * L2;
-    double* gs = smem + (size_t)warp * desc_warp_doubles(bs.n_max, L2, bs.NvL2);
+    const int Nv = bs.Nv;
+    double* gs = smem + (size_t)warp * desc_warp_doubles(bs.n_max, L2, Nv);
     double* ys = gs + 32 * GS;
     double* As = ys + 32 * YS;
-    int* sjs = reinterpret_cast<int*>(As + bs.NvL2);
+    int* sjs = reinterpret_cast<int*>(As + Nv * AS);
 
     const int k = atom_of_row[row0 + local];
     const AtomS me = load_atom(atoms + k);
     const int cnt = nbr_cnt[k];
-    for (int c = lane; c < bs.NvL2; c += 32) As[c] = 0.0;
+    for (int c = lane; c < Nv * AS; c += 32) As[c] = 0.0;
 
     for (int base = 0; base < cnt; base += 32) {
         const int nact = min(32, cnt - base);
@@ -58,14 +73,27 @@ k_descriptor(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const 
         }
         sjs[lane] = sj;
         __syncwarp();
-        for (int s = 0; s < bs.S; s++) {
-            if (!__any_sync(kFull, sj == s)) continue;
-            for (int c = lane; c < nL2; c += 32) {
-                const int n = c / L2, lm = c - n * L2;
-                double acc = 0.0;
-                for (int jj = 0; jj < nact; jj++)
-                    if (sjs[jj] == s) acc = fma(gs[jj * GS + n], ys[jj * YS + lm], acc);
-                As[s * nL2 + c] += acc;
+        // A += G^T Y on the tensor pipe.  Fragment roles (m8n8k4): A-operand (row nu = 8mb+g8, col j = k0+t4),
+        // B-operand (row j = k0+t4, col lm = 8nb+g8), C (row nu = 8mb+g8, cols lm = 8nb+2t4, +1).
+        for (int mb = 0; mb * 8 < Nv; mb++) {
+            const int nu = mb * 8 + g8;
+            const int s_nu = (nu < Nv) ? nu / bs.n_max : -2;
+            const int n_nu = nu - s_nu * bs.n_max;
+#pragma unroll 1
+            for (int nb = 0; nb * 8 < L2; nb++) {
+                const int lmb = nb * 8 + g8;
+                double c0 = 0.0, c1 = 0.0;
+                for (int k0 = 0; k0 < nact; k0 += 4) {
+                    const int j = k0 + t4;  // < 32 always; lanes >= nact carry sjs = -1
+                    const double a = (sjs[j] == s_nu) ? gs[j * GS + n_nu] : 0.0;
+                    const double b = (j < nact && lmb < L2) ? ys[j * YS + lmb] : 0.0;
+                    dmma884_d(c0, c1, a, b);
+                }
+                const int lm0 = nb * 8 + 2 * t4;
+                if (nu < Nv) {
+                    if (lm0 < L2) As[nu * AS + lm0] += c0;
+                    if (lm0 + 1 < L2) As[nu * AS + lm0 + 1] += c1;
+                }
             }
         }
         __syncwarp();
@@ -73,38 +101,46 @@ k_descriptor(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const 
 
     if (A_out) {
         double* arow = A_out + (size_t)local * bs.NvL2;
-        for (int c = lane; c < bs.NvL2; c += 32) arow[c] = As[c];
+        for (int c = lane; c < bs.NvL2; c += 32) {
+            const int nu = c / L2;
+            arow[c] = As[nu * AS + (c - nu * L2)];
+        }
     }
 
-    // B2 contraction: B[nu1<=nu2, l] = sum_m A[nu1,l,m] A[nu2,l,m]; first pass for ||B||, second writes B^
+    // B2 contraction, one (nu1,nu2) pair per lane, all l at once.
     const GroupDev gd = groups[gid[k]];
+    const int npairs = gd.P / L;
     double n2 = 0.0;
-    for (int p = lane; p < gd.P; p += 32) {
-        const int t = __ldg(gd.table + p);
-        const int v1 = t & 255, v2 = (t >> 8) & 255, l = t >> 16;
-        const double* a1 = As + v1 * L2 + l * l;
-        const double* a2 = As + v2 * L2 + l * l;
-        double b = 0.0;
-        for (int i = 0; i <= 2 * l; i++) b = fma(a1[i], a2[i], b);
-        n2 = fma(b, b, n2);
+    for (int q = lane; q < npairs; q += 32) {
+        const int t = __ldg(gd.table + q);
+        const double* a1 = As + (t & 255) * AS;
+        const double* a2 = As + (t >> 8) * AS;
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+            double b = 0.0;
+#pragma unroll
+            for (int i = l * l; i < (l + 1) * (l + 1); i++) b = fma(a1[i], a2[i], b);
+            n2 = fma(b, b, n2);
+        }
     }
     n2 = warp_sum(n2);
     const double nrm = sqrt(n2);
     const double inv = (nrm > 0.0) ? 1.0 / nrm : 0.0;  // empty neighbourhood: B^ = 0 (R8)
     const int orow = out_map ? out_map[k] : local;
     double* brow = bh_out + (size_t)orow * ld;
-    const int pend = min(gd.K, ld);
-    for (int p = lane; p < pend; p += 32) {
-        double b = 0.0;
-        if (p < gd.P) {
-            const int t = __ldg(gd.table + p);
-            const int v1 = t & 255, v2 = (t >> 8) & 255, l = t >> 16;
-            const double* a1 = As + v1 * L2 + l * l;
-            const double* a2 = As + v2 * L2 + l * l;
-            for (int i = 0; i <= 2 * l; i++) b = fma(a1[i], a2[i], b);
+    for (int q = lane; q < npairs; q += 32) {
+        const int t = __ldg(gd.table + q);
+        const double* a1 = As + (t & 255) * AS;
+        const double* a2 = As + (t >> 8) * AS;
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+            double b = 0.0;
+#pragma unroll
+            for (int i = l * l; i < (l + 1) * (l + 1); i++) b = fma(a1[i], a2[i], b);
+            brow[q * L + l] = b * inv;
         }
-        brow[p] = b * inv;
     }
+    for (int p = gd.P + lane; p < min(gd.K, ld); p += 32) brow[p] = 0.0;  // zero padding up to K
     if (lane == 0) nrm_out[orow] = nrm;
 }
 
@@ -113,7 +149,7 @@ static void launch_descriptor(Launcher& L, const Grid& g, const Basis& bs, const
                               int mmax, const GroupDev* groups, int row0, int nrows, double* bh_out, int ld,
                               double* nrm_out, const int* out_map, bool write_A) {
     constexpr int L2 = (LMAX + 1) * (LMAX + 1);
-    const size_t smem = sizeof(double) * kDescWarps * (size_t)desc_warp_doubles(bs.n_max, L2, bs.NvL2);
+    const size_t smem = sizeof(double) * kDescWarps * (size_t)desc_warp_doubles(bs.n_max, L2, bs.Nv);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         cudaFuncSetAttribute(k_descriptor<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

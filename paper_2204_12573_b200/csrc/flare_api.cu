@@ -145,12 +145,6 @@ std::vector<double> pack_matrix(const double* m, int P, const std::vector<int>& 
 int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
     const Basis& bs = c->bs;
     const int S = bs.S, L = bs.l_max + 1, Nv = bs.Nv, P = bs.P;
-    // dense component table (nu1, nu2>=nu1, l) in the order of R4
-    std::vector<int> dense_table;
-    dense_table.reserve(P);
-    for (int v1 = 0; v1 < Nv; v1++)
-        for (int v2 = v1; v2 < Nv; v2++)
-            for (int l = 0; l < L; l++) dense_table.push_back(v1 | (v2 << 8) | (l << 16));
     c->n_groups = c->sparse ? S * (1 << S) : S;
     c->groups.assign(c->n_groups, GroupDesc{});
     std::vector<GroupDev> gdev(c->n_groups);
@@ -159,16 +153,20 @@ int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
     for (int gi = 0; gi < c->n_groups; gi++) {
         const int s = c->sparse ? gi / (1 << S) : gi;
         const unsigned mask = c->sparse ? (unsigned)(gi % (1 << S)) : ((1u << S) - 1u);
-        // components whose both radial channels belong to species present in the mask
-        std::vector<int> comp, table;
-        for (int p = 0; p < P; p++) {
-            const int t = dense_table[p];
-            const int s1 = (t & 255) / bs.n_max, s2 = ((t >> 8) & 255) / bs.n_max;
-            if (((mask >> s1) & 1u) && ((mask >> s2) & 1u)) { comp.push_back(p); table.push_back(t); }
-        }
+        // (nu1 <= nu2) pairs whose radial channels both belong to species present in the mask;
+        // component p = q*L + l keeps the dense order (nu1, nu2, l) of R4 restricted to those pairs
+        std::vector<int> comp, table, lut((size_t)Nv * Nv, -1);
+        for (int v1 = 0, dense_q = 0; v1 < Nv; v1++)
+            for (int v2 = v1; v2 < Nv; v2++, dense_q++) {
+                const int s1 = v1 / bs.n_max, s2 = v2 / bs.n_max;
+                if (!(((mask >> s1) & 1u) && ((mask >> s2) & 1u))) continue;
+                lut[(size_t)v1 * Nv + v2] = lut[(size_t)v2 * Nv + v1] = (int)table.size();
+                table.push_back(v1 | (v2 << 8));
+                for (int l = 0; l < L; l++) comp.push_back(dense_q * L + l);
+            }
         GroupDesc& gd = c->groups[gi];
         gd.P = (int)comp.size();
-        if (gd.P == 0) { gdev[gi] = GroupDev{0, 0, 0, 0, nullptr}; continue; }
+        if (gd.P == 0) { gdev[gi] = GroupDev{0, 0, 0, 0, nullptr, nullptr}; continue; }
         gd.K = round_up(gd.P, 16);
         choose_tiles(gd.K, gd.nb, gd.ntn);
         const int rows = gd.ntn * gd.nb * 8;
@@ -185,7 +183,10 @@ int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
         rc = upload(c, table, &dt);
         if (rc) return rc;
         gd.table = dt;
-        gdev[gi] = GroupDev{gd.P, gd.K, gd.ntn, 0, gd.table};
+        rc = upload(c, lut, &dt);
+        if (rc) return rc;
+        gd.lut = dt;
+        gdev[gi] = GroupDev{gd.P, gd.K, gd.ntn, 0, gd.table, gd.lut};
         c->max_ntn = std::max(c->max_ntn, gd.ntn);
         c->ld = std::max(c->ld, gd.K);
     }

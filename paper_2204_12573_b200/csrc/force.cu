@@ -16,12 +16,42 @@ namespace flare {
 
 constexpr int kBpWarps = 4;
 
-__host__ __device__ inline int bp_warp_doubles(int n_max, int NvL2, int ld) {
-    // A, G : NvL2 each; c : ld; per-lane radial values g, dg : 2 * n_max * 32
-    return 2 * NvL2 + ld + 2 * n_max * 32;
+__host__ __device__ inline int bp_warp_doubles(int S, int Nv, int L2, int nmaxp, int ld) {
+    // A[Nv][L2|1], c[ld], G^T[S][L2][nmaxp]
+    return (Nv * (L2 | 1) + ld + S * L2 * nmaxp + 1) & ~1;  // even: keeps every warp's G^T 16-byte aligned
 }
 
-template <int LMAX>
+__device__ __forceinline__ void dmma884_f(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// g[n] = T_n(x) f_c(r), dg[n] = d g[n]/dr for n < n_max, zero above; fully unrolled so that g/dg stay in registers
+template <int NMAXP>
+__device__ __forceinline__ void radial_fixed(int n_max, double r, double rc, double (&gv)[NMAXP], double (&dgv)[NMAXP]) {
+    const double inv_rc = 1.0 / rc;
+    const double q = r * inv_rc;
+    const double x = 2.0 * q - 1.0;
+    double sn, cs;
+    sincospi(q, &sn, &cs);
+    const double fc = 0.5 * (1.0 + cs);
+    const double dfc = -0.5 * kPi * inv_rc * sn;
+    const double dxdr = 2.0 * inv_rc;
+    double t0 = 1.0, t1 = x, u0 = 0.0, u1 = 1.0;
+#pragma unroll
+    for (int n = 0; n < NMAXP; n++) {
+        const bool on = n < n_max;
+        gv[n] = on ? t0 * fc : 0.0;
+        dgv[n] = on ? dxdr * ((double)n * u0) * fc + t0 * dfc : 0.0;
+        const double t2 = 2.0 * x * t1 - t0;
+        t0 = t1; t1 = t2;
+        const double u2 = 2.0 * x * u1 - u0;
+        u0 = u1; u1 = u2;
+    }
+}
+
+template <int LMAX, int NMAXP>
 __global__ void __launch_bounds__(kBpWarps * 32)
 k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
            const int* __restrict__ nbr_idx, int mmax, const int* __restrict__ atom_of_row,
@@ -29,16 +59,19 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
            const double* __restrict__ A_in, const double* __restrict__ Bh, const double* __restrict__ W,
            const double* __restrict__ nrm_in, const double* __restrict__ part, int ld, int chunk_cap, int max_ntn,
            int want_variance, double* __restrict__ pairf, double* __restrict__ e_s, double* __restrict__ v_s) {
-    constexpr int L2 = (LMAX + 1) * (LMAX + 1);
-    extern __shared__ double smem[];
+    constexpr int L = LMAX + 1;
+    constexpr int L2 = L * L;
+    constexpr int AS = L2 | 1;
+    constexpr int NBL = (2 * LMAX + 1 + 7) / 8;  // n8 blocks needed for the widest m range
+    extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int local = blockIdx.x * kBpWarps + warp;
     if (local >= nrows) return;
-    double* As = smem + (size_t)warp * bp_warp_doubles(bs.n_max, bs.NvL2, ld);
-    double* Gs = As + bs.NvL2;
-    double* cs = Gs + bs.NvL2;
-    double* gl = cs + ld;                 // [n_max][32] this lane's g~_n
-    double* dgl = gl + bs.n_max * 32;     // [n_max][32] this lane's d g~_n / dr
+    const int g8 = lane >> 2, t4 = lane & 3;
+    const int Nv = bs.Nv;
+    double* Gt = smem + (size_t)warp * bp_warp_doubles(bs.S, Nv, L2, NMAXP, ld);  // [S][L2][NMAXP], 16-byte aligned
+    double* As = Gt + bs.S * L2 * NMAXP;
+    double* cs = As + Nv * AS;
 
     const int k = atom_of_row[row0 + local];
     const GroupDev gd = groups[gid[k]];
@@ -52,51 +85,66 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
     const double two_inv = (nrm > 0.0) ? 2.0 / nrm : 0.0;
     if (lane == 0) { e_s[k] = E; v_s[k] = V; }
 
-    // ---- stage A and c = dE/dB
+    // ---- stage A, zero G^T, stage c = dE/dB with the diagonal pairs pre-doubled (the 1 + delta factor)
     const double* arow = A_in + (size_t)local * bs.NvL2;
-    for (int c = lane; c < bs.NvL2; c += 32) { As[c] = arow[c]; Gs[c] = 0.0; }
+    for (int c = lane; c < bs.NvL2; c += 32) {
+        const int nu = c / L2;
+        As[nu * AS + (c - nu * L2)] = arow[c];
+    }
+    for (int c = lane; c < bs.S * L2 * NMAXP; c += 32) Gt[c] = 0.0;
     const double* wrow = W + (size_t)local * ld;
     const double* brow = Bh + (size_t)local * ld;
-    for (int p = lane; p < gd.P; p += 32) cs[p] = two_inv * (wrow[p] - E * brow[p]);
+    for (int p = lane; p < gd.P; p += 32) {
+        const int t = __ldg(gd.table + p / L);
+        const double dbl = ((t & 255) == (t >> 8)) ? 2.0 : 1.0;
+        cs[p] = dbl * two_inv * (wrow[p] - E * brow[p]);
+    }
     __syncwarp();
 
-    // ---- G[nu1,lm] = sum_nu2 c_p (1+delta) A[nu2,lm]: lanes own (nu1,lm); loop the group's components.
-    // The component table is ordered (nu1, nu2>=nu1, l), so for a fixed (nu, l) the components with
-    // nu as FIRST index are contiguous in nu2 and those with nu as SECOND index are found by table walk;
-    // with P up to a few thousand a direct walk over p per lane would be wasteful, so each lane walks
-    // only the (nu2) partners of its own (nu1, l) through the closed-form index of the dense ordering
-    // when the group is dense, and through the table otherwise.
-    {
-        const int Nv = bs.Nv;
-        const int L = LMAX + 1;
-        for (int c = lane; c < bs.NvL2; c += 32) {
-            const int v1 = c / L2, lm = c - v1 * L2;
-            int l = 0;
-            while ((l + 1) * (l + 1) <= lm) l++;
-            double acc = 0.0;
-            if (gd.P == bs.P) {
-                // dense ordering: p(a<=b, l) = (a*Nv - a(a-1)/2 + (b-a))*L + l
-                for (int v2 = 0; v2 < Nv; v2++) {
-                    const int a = min(v1, v2), b = max(v1, v2);
-                    const int p = (a * Nv - (a * (a - 1)) / 2 + (b - a)) * L + l;
-                    const double w = (v1 == v2) ? 2.0 : 1.0;
-                    acc = fma(w * cs[p], As[v2 * L2 + lm], acc);
-                }
-            } else {
-                for (int p = 0; p < gd.P; p++) {
-                    const int t = __ldg(gd.table + p);
-                    const int a = t & 255, b = (t >> 8) & 255, ll = t >> 16;
-                    if (ll != l) continue;
-                    if (a == v1) acc = fma((a == b ? 2.0 : 1.0) * cs[p], As[b * L2 + lm], acc);
-                    else if (b == v1) acc = fma(cs[p], As[a * L2 + lm], acc);
+    // ---- G[nu1, (l,m)] = sum_nu2 C_l[nu1,nu2] A[nu2,(l,m)] with C_l[nu1,nu2] = c[q(nu1,nu2) L + l]: per l a small
+    // symmetric-matrix product on the tensor pipe.  A-operand (row nu1 = 8mb+g8, col nu2 = k0+t4),
+    // B-operand (row nu2 = k0+t4, col m = 8nb+g8), C (row nu1, cols m = 8nb+2t4, +1).
+    for (int mb = 0; mb * 8 < Nv; mb++) {
+        const int nu1 = mb * 8 + g8;
+        double acc[L][NBL][2];
+#pragma unroll
+        for (int l = 0; l < L; l++)
+#pragma unroll
+            for (int nb = 0; nb < NBL; nb++) { acc[l][nb][0] = 0.0; acc[l][nb][1] = 0.0; }
+        for (int k0 = 0; k0 < Nv; k0 += 4) {
+            const int nu2 = k0 + t4;
+            const bool in = nu1 < Nv && nu2 < Nv;
+            const int q = in ? __ldg(gd.lut + nu1 * Nv + nu2) : -1;
+            const double* a2 = As + (nu2 < Nv ? nu2 : 0) * AS;
+#pragma unroll
+            for (int l = 0; l < L; l++) {
+                const double a = (q >= 0) ? cs[q * L + l] : 0.0;
+#pragma unroll
+                for (int nb = 0; nb < NBL; nb++) {
+                    if (nb * 8 < 2 * l + 1) {
+                        const int m = nb * 8 + g8;
+                        const double b = (nu2 < Nv && m < 2 * l + 1) ? a2[l * l + m] : 0.0;
+                        dmma884_f(acc[l][nb][0], acc[l][nb][1], a, b);
+                    }
                 }
             }
-            Gs[c] = acc;
+        }
+        if (nu1 < Nv) {
+            const int s1 = nu1 / bs.n_max, n1 = nu1 - s1 * bs.n_max;
+            double* gt = Gt + (size_t)s1 * L2 * NMAXP + n1;
+#pragma unroll
+            for (int l = 0; l < L; l++)
+#pragma unroll
+                for (int nb = 0; nb < NBL; nb++) {
+                    const int m = nb * 8 + 2 * t4;
+                    if (m < 2 * l + 1) gt[(l * l + m) * NMAXP] = acc[l][nb][0];
+                    if (m + 1 < 2 * l + 1) gt[(l * l + m + 1) * NMAXP] = acc[l][nb][1];
+                }
         }
     }
     __syncwarp();
 
-    // ---- per-pair forces: lanes over neighbours
+    // ---- per-pair forces f_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj): lanes over neighbours
     const AtomS me = load_atom(atoms + k);
     const int cnt = nbr_cnt[k];
     for (int base = 0; base < cnt; base += 32) {
@@ -109,16 +157,20 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
             const double r = sqrt(dx * dx + dy * dy + dz * dz);
             const double ir = 1.0 / r;
             const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-            radial_basis<true>(bs.n_max, r, bs.rc[me.type * bs.S + o.type],
-                               [&](int n, double gv, double dgv) { gl[n * 32 + lane] = gv; dgl[n * 32 + lane] = dgv; });
-            const double* Gj = Gs + o.type * bs.n_max * L2;
+            double gr[NMAXP], dgr[NMAXP];
+            radial_fixed<NMAXP>(bs.n_max, r, bs.rc[me.type * bs.S + o.type], gr, dgr);
+            const double* Gj = Gt + (size_t)o.type * L2 * NMAXP;
             double srad = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
             real_ylm<LMAX, true>(yn, ux, uy, uz, [&](int lm, double Y, double gx, double gy, double gz) {
+                const double2* gp = reinterpret_cast<const double2*>(Gj + lm * NMAXP);
                 double hr = 0.0, hg = 0.0;  // sum_n G[n,lm] dg_n  and  sum_n G[n,lm] g_n
-                for (int n = 0; n < bs.n_max; n++) {
-                    const double Gv = Gj[n * L2 + lm];
-                    hr = fma(Gv, dgl[n * 32 + lane], hr);
-                    hg = fma(Gv, gl[n * 32 + lane], hg);
+#pragma unroll
+                for (int n2 = 0; n2 < NMAXP / 2; n2++) {
+                    const double2 Gv = gp[n2];
+                    hr = fma(Gv.x, dgr[2 * n2], hr);
+                    hr = fma(Gv.y, dgr[2 * n2 + 1], hr);
+                    hg = fma(Gv.x, gr[2 * n2], hg);
+                    hg = fma(Gv.y, gr[2 * n2 + 1], hg);
                 }
                 srad = fma(hr, Y, srad);
                 vx = fma(hg, gx, vx);
@@ -135,17 +187,18 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
     }
 }
 
-template <int LMAX>
+template <int LMAX, int NMAXP>
 static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
                             int mmax, const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
                             bool want_variance) {
-    const size_t smem = sizeof(double) * kBpWarps * (size_t)bp_warp_doubles(bs.n_max, bs.NvL2, ld);
+    constexpr int L2 = (LMAX + 1) * (LMAX + 1);
+    const size_t smem = sizeof(double) * kBpWarps * (size_t)bp_warp_doubles(bs.S, bs.Nv, L2, NMAXP, ld);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(k_backprop<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_backprop<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    L.launch(k_backprop<LMAX>, dim3((nrows + kBpWarps - 1) / kBpWarps), dim3(kBpWarps * 32), smem, g, bs, yn,
+    L.launch(k_backprop<LMAX, NMAXP>, dim3((nrows + kBpWarps - 1) / kBpWarps), dim3(kBpWarps * 32), smem, g, bs, yn,
              (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const unsigned char*)ws.gid, groups, row0, nrows, (const double*)ws.A,
              (const double*)ws.Bh, (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap,
@@ -156,13 +209,18 @@ void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, 
                   const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
                   bool want_variance) {
     if (nrows <= 0) return;
+#define FLARE_CASE(LM)                                                                                                \
+    case LM:                                                                                                          \
+        if (bs.n_max <= 8)                                                                                            \
+            launch_backprop<LM, 8>(L, g, bs, yn, ws, mmax, groups, row0, nrows, ld, chunk_cap, max_ntn, want_variance); \
+        else                                                                                                          \
+            launch_backprop<LM, 16>(L, g, bs, yn, ws, mmax, groups, row0, nrows, ld, chunk_cap, max_ntn, want_variance); \
+        break;
     switch (bs.l_max) {
-#define FLARE_CASE(LM) \
-    case LM: launch_backprop<LM>(L, g, bs, yn, ws, mmax, groups, row0, nrows, ld, chunk_cap, max_ntn, want_variance); break;
         FLARE_CASE(0) FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6)
-#undef FLARE_CASE
         default: break;
     }
+#undef FLARE_CASE
 }
 
 // ------------------------------------------------------------------ a7: atomics-free gather

@@ -80,7 +80,8 @@ struct GroupDesc {
     int ntn = 0;          // tiles along N per matrix
     const double* beta = nullptr;   // device [ntn*8*nb][K] padded, symmetric
     const double* sigma = nullptr;  // same or nullptr
-    const int* table = nullptr;     // device [P]: component p -> nu1 | nu2<<8 | l<<16
+    const int* table = nullptr;     // device [P/(l_max+1)]: pair q -> nu1 | nu2<<8; component p = q*(l_max+1) + l
+    const int* lut = nullptr;       // device [Nv*Nv]: (nu1,nu2) -> pair q (symmetric), -1 if not in the group
 };
 
 // What the per-atom kernels need to know about a group (device array indexed by group id).
@@ -89,7 +90,8 @@ struct GroupDev {
     int K;
     int ntn;
     int pad_;
-    const int* table;
+    const int* table;  // pair table, see GroupDesc
+    const int* lut;    // pair lookup, see GroupDesc
 };
 
 // stage entry points (each enqueues kernels through the Launcher)
