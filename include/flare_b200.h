@@ -61,8 +61,9 @@ enum {
     FLARE_OPT_CHUNK_ATOMS = 2,   /* atoms per chunk of the descriptor/quadratic-form/back-prop stage
                                     ("dividing atoms into batches"); 0 = automatic (default) */
     FLARE_OPT_TIMING = 3,        /* 1: bracket every kernel phase with CUDA events (flare_get_timings) */
-    FLARE_OPT_SPECIES_SPARSE = 4 /* 1: skip descriptor blocks of absent neighbour species;
-                                    exact; default 0 in this version */
+    FLARE_OPT_SPECIES_SPARSE = 4 /* 1 (default when S * 2^S <= 64): atoms are grouped by the set of neighbour species
+                                    present and the descriptor blocks of absent species are skipped in a2-a6
+                                    ("420 to 112"); exact.  0: every atom uses all P components. */
 };
 
 /* Kernel phases reported by flare_get_timings, in this order. */

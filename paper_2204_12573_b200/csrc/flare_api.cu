@@ -31,9 +31,18 @@ struct flare_ctx {
     YNorm yn{};
     std::vector<double> mass;
     bool has_sigma = false;
-    // model on device
+    // model on device: two group sets are built at create time, [0] dense (one group per central species),
+    // [1] species-sparse (one group per (central species, neighbour-species mask)); the active one
+    // is mirrored into groups / d_groups / n_groups / max_ntn / ld
     std::vector<void*> dev_allocs;
-    std::vector<GroupDesc> groups;  // host copy (device pointers inside)
+    struct GroupSet {
+        std::vector<GroupDesc> groups;        // host copy (device pointers inside)
+        std::vector<std::vector<int>> comps;  // per group: dense component index of each compacted component
+        GroupDev* d_groups = nullptr;
+        int n_groups = 0, max_ntn = 0, ld = 0;
+    } sets[2];
+    bool have_sparse = false;
+    std::vector<GroupDesc> groups;
     GroupDev* d_groups = nullptr;
     int n_groups = 0;
     int max_ntn = 0;
@@ -142,17 +151,30 @@ std::vector<double> pack_matrix(const double* m, int P, const std::vector<int>& 
     return out;
 }
 
-int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
+void activate_groups(flare_ctx* c, int sparse) {
+    const flare_ctx::GroupSet& gs = c->sets[sparse];
+    c->sparse = sparse;
+    c->groups = gs.groups;
+    c->d_groups = gs.d_groups;
+    c->n_groups = gs.n_groups;
+    c->max_ntn = gs.max_ntn;
+    c->ld = gs.ld;
+    c->bs.Pld = gs.ld;
+}
+
+int build_groups(flare_ctx* c, const double* beta, const double* sigma, int sparse) {
     const Basis& bs = c->bs;
     const int S = bs.S, L = bs.l_max + 1, Nv = bs.Nv, P = bs.P;
-    c->n_groups = c->sparse ? S * (1 << S) : S;
-    c->groups.assign(c->n_groups, GroupDesc{});
-    std::vector<GroupDev> gdev(c->n_groups);
-    c->max_ntn = 0;
-    c->ld = 16;
-    for (int gi = 0; gi < c->n_groups; gi++) {
-        const int s = c->sparse ? gi / (1 << S) : gi;
-        const unsigned mask = c->sparse ? (unsigned)(gi % (1 << S)) : ((1u << S) - 1u);
+    flare_ctx::GroupSet& set = c->sets[sparse];
+    set.n_groups = sparse ? S * (1 << S) : S;
+    set.groups.assign(set.n_groups, GroupDesc{});
+    set.comps.assign(set.n_groups, {});
+    std::vector<GroupDev> gdev(set.n_groups);
+    set.max_ntn = 0;
+    set.ld = 16;
+    for (int gi = 0; gi < set.n_groups; gi++) {
+        const int s = sparse ? gi / (1 << S) : gi;
+        const unsigned mask = sparse ? (unsigned)(gi % (1 << S)) : ((1u << S) - 1u);
         // (nu1 <= nu2) pairs whose radial channels both belong to species present in the mask;
         // component p = q*L + l keeps the dense order (nu1, nu2, l) of R4 restricted to those pairs
         std::vector<int> comp, table, lut((size_t)Nv * Nv, -1);
@@ -164,8 +186,9 @@ int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
                 table.push_back(v1 | (v2 << 8));
                 for (int l = 0; l < L; l++) comp.push_back(dense_q * L + l);
             }
-        GroupDesc& gd = c->groups[gi];
+        GroupDesc& gd = set.groups[gi];
         gd.P = (int)comp.size();
+        set.comps[gi] = comp;
         if (gd.P == 0) { gdev[gi] = GroupDev{0, 0, 0, 0, nullptr, nullptr}; continue; }
         gd.K = round_up(gd.P, 16);
         choose_tiles(gd.K, gd.nb, gd.ntn);
@@ -187,10 +210,10 @@ int build_groups(flare_ctx* c, const double* beta, const double* sigma) {
         if (rc) return rc;
         gd.lut = dt;
         gdev[gi] = GroupDev{gd.P, gd.K, gd.ntn, 0, gd.table, gd.lut};
-        c->max_ntn = std::max(c->max_ntn, gd.ntn);
-        c->ld = std::max(c->ld, gd.K);
+        set.max_ntn = std::max(set.max_ntn, gd.ntn);
+        set.ld = std::max(set.ld, gd.K);
     }
-    return upload(c, gdev, &c->d_groups);
+    return upload(c, gdev, &set.d_groups);
 }
 
 // ---------------------------------------------------------------- workspace layout
@@ -391,14 +414,16 @@ int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_m
             if (m > 0) k *= std::sqrt(2.0);
             c->yn.k[l * (l + 1) / 2 + m] = k;
         }
-    int rc = build_groups(c, beta, sigma);
+    int rc = build_groups(c, beta, sigma, 0);
+    c->have_sparse = n_species * (1 << n_species) <= kMaxGroups;
+    if (rc == FLARE_OK && c->have_sparse) rc = build_groups(c, beta, sigma, 1);
+    if (rc == FLARE_OK) activate_groups(c, c->have_sparse ? 1 : 0);  // species-sparse evaluation is the default
     if (rc == FLARE_OK) {
         void* d = nullptr;
         if (cudaMalloc(&d, sizeof(double) * kMaxSpecies) != cudaSuccess) rc = FLARE_ERR_CUDA;
         else { c->dev_allocs.push_back(d); c->d_accel = (double*)d; }
     }
     if (rc != FLARE_OK) { flare_destroy(c); return rc; }
-    bs.Pld = c->ld;
     c->h_accel.assign(kMaxSpecies, 0.0);
     *out = c;
     return FLARE_OK;
@@ -432,7 +457,10 @@ int flare_set_option(flare_ctx* c, int option, int64_t value) {
             c->timing = value ? 1 : 0;
             return FLARE_OK;
         case FLARE_OPT_SPECIES_SPARSE:
-            if (value) return fail(c, FLARE_ERR_UNSUPPORTED, "species-sparse mode is not available in this version");
+            if (value && !c->have_sparse)
+                return fail(c, FLARE_ERR_UNSUPPORTED, "species-sparse mode needs S * 2^S <= 64 groups");
+            activate_groups(c, value ? 1 : 0);
+            c->n = -1;
             return FLARE_OK;
         default:
             return fail(c, FLARE_ERR_INVALID_ARG, "unknown option");
@@ -672,16 +700,18 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
     if (rc) return rc;
     if (!c->have_grid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
     if (!bhat || !nrm) return fail(c, FLARE_ERR_INVALID_ARG, "bad output arrays");
-    if (c->sparse) return fail(c, FLARE_ERR_UNSUPPORTED, "descriptor hook needs dense mode");
     rc = flare_check(c);
     if (rc) return rc;
     const int n = (int)c->n;
     const int P = c->bs.P;
     std::vector<AtomS> h_atoms((size_t)n);
     std::vector<int> h_aor((size_t)n);
+    std::vector<unsigned char> h_gid((size_t)n);
     if (n == 0) return FLARE_OK;
     FLARE_CUDA(c, cudaMemcpy(h_atoms.data(), c->ws.atoms, sizeof(AtomS) * n, cudaMemcpyDeviceToHost));
     FLARE_CUDA(c, cudaMemcpy(h_aor.data(), c->ws.atom_of_row, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    FLARE_CUDA(c, cudaMemcpy(h_gid.data(), c->ws.gid, n, cudaMemcpyDeviceToHost));
+    const auto& comps = c->sets[c->sparse].comps;
     Launcher L;
     L.stream = c->stream;
     L.launch_count = &c->launches;
@@ -697,8 +727,12 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
         FLARE_CUDA(c, cudaMemcpyAsync(hn.data(), c->ws.nrm, sizeof(double) * nrows, cudaMemcpyDeviceToHost, c->stream));
         FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
         for (int r = 0; r < nrows; r++) {
-            const int i = h_atoms[h_aor[row0 + r]].orig;
-            memcpy(bhat + (size_t)i * P, hb.data() + (size_t)r * c->ld, sizeof(double) * P);
+            const int k = h_aor[row0 + r];
+            const int i = h_atoms[k].orig;
+            const std::vector<int>& comp = comps[h_gid[k]];  // compacted -> dense component (identity in dense mode)
+            double* dst = bhat + (size_t)i * P;
+            for (int p = 0; p < P; p++) dst[p] = 0.0;
+            for (size_t q = 0; q < comp.size(); q++) dst[comp[q]] = hb[(size_t)r * c->ld + q];
             nrm[i] = hn[r];
         }
     }

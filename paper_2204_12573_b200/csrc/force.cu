@@ -84,6 +84,7 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
     const double nrm = nrm_in[local];
     const double two_inv = (nrm > 0.0) ? 2.0 / nrm : 0.0;
     if (lane == 0) { e_s[k] = E; v_s[k] = V; }
+    if (gd.P == 0) return;  // no neighbours (R8): E = V = 0 and no pair forces; the group has no tables
 
     // ---- stage A, zero G^T, stage c = dE/dB with the diagonal pairs pre-doubled (the 1 + delta factor)
     const double* arow = A_in + (size_t)local * bs.NvL2;

@@ -109,7 +109,8 @@ class Flare:
     """One model context bound to one CUDA device (flare_create ... flare_destroy)."""
 
     def __init__(self, mass, n_max: int, l_max: int, r_cut, beta, sigma=None, device: int = 0,
-                 max_neighbors: int | None = None, chunk_atoms: int | None = None, timing: bool = False):
+                 max_neighbors: int | None = None, chunk_atoms: int | None = None, timing: bool = False,
+                 species_sparse: bool | None = None):
         import torch  # device memory + stream only
 
         self._torch = torch
@@ -142,6 +143,8 @@ class Flare:
             self.set_option(OPT_CHUNK_ATOMS, chunk_atoms)
         if timing:
             self.set_option(OPT_TIMING, 1)
+        if species_sparse is not None:
+            self.set_option(OPT_SPECIES_SPARSE, 1 if species_sparse else 0)
 
     # ------------------------------------------------------------------ plumbing
     def _check(self, rc: int):

@@ -81,9 +81,11 @@ def test_config1_full(oracle, torch, flare):
         assert abs(nrm[i] - n0) < 1e-12 * n0
 
 
-def test_config2_full(oracle, torch, flare):
+@pytest.mark.parametrize("sparse", [True, False])
+def test_config2_full(oracle, torch, flare, sparse):
     s = w.config2()
-    ctx, got, want = assert_parity(oracle, torch, flare, s, nbr_method=0)
+    ctx, got, want = assert_parity(oracle, torch, flare, s, nbr_method=0, species_sparse=sparse)
+    assert ctx.get_option(4) == int(sparse)
     bh, nrm = ctx.descriptors()
     for i in (0, 500, 863, 864, 1263):  # Pt bulk, Pt surface, H
         _, _, Bh, n0 = oracle.descriptor(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, i)
@@ -94,10 +96,39 @@ def test_config2_full(oracle, torch, flare):
 # ----------------------------------------------------------------------------- basis sizes, several tiles + ragged tails
 
 
-@pytest.mark.parametrize("n_max,l_max", [(1, 0), (3, 1), (4, 2), (7, 3), (3, 4), (2, 5), (2, 6), (5, 6)])
-def test_basis_sizes_on_a_small_tile(oracle, torch, flare, n_max, l_max):
+@pytest.mark.parametrize("sparse", [True, False])
+@pytest.mark.parametrize("n_max,l_max", [(1, 0), (3, 1), (4, 2), (7, 3), (3, 4), (2, 5), (2, 6), (5, 6), (9, 2)])
+def test_basis_sizes_on_a_small_tile(oracle, torch, flare, n_max, l_max, sparse):
     s = w.tile_like_c3(6, 3, n_max=n_max, l_max=l_max)  # 216 Pt + 18 H
-    assert_parity(oracle, torch, flare, s)
+    assert_parity(oracle, torch, flare, s, species_sparse=sparse)
+
+
+def test_species_sparse_is_the_default_and_matches_dense(torch, flare):
+    """skipping the blocks of absent neighbour species is exact; here against the dense evaluation."""
+    s = w.tile_like_c3(12, 6)
+    c1, e1, f1, v1 = gpu_compute(torch, flare, s)
+    assert c1.get_option(4) == 1
+    c0, e0, f0, v0 = gpu_compute(torch, flare, s, species_sparse=False)
+    assert np.abs(e1 - e0).max() < 1e-13 and np.abs(f1 - f0).max() < 1e-12 and np.abs(v1 - v0).max() < 1e-16
+    b1, n1 = c1.descriptors()
+    b0, n0 = c0.descriptors()
+    assert np.abs(b1 - b0).max() < 1e-14 and np.abs(n1 - n0).max() < 1e-12 * n0.max()
+
+
+def test_three_species_sparse(oracle, torch, flare):
+    """Three species: 24 (species, mask) groups; random species on a jittered fcc lattice."""
+    rng = np.random.default_rng(41)
+    pos, _, box, pbc = w.fcc_bulk(4, w.A_PT, 0.05, rng)
+    types = rng.integers(0, 3, pos.shape[0]).astype(np.int32)
+    types[:40] = 0  # some single-species neighbourhoods are unlikely in a random alloy; keep the mix anyway
+    n_max, l_max, S = 3, 2, 3
+    r_cut = np.array([[4.25, 3.6, 3.0], [3.6, 3.6, 3.0], [3.0, 3.0, 3.0]])
+    P = w.num_descriptors(S, n_max, l_max)
+    s = w.System("three", pos, types, box, pbc, np.array([195.0, 100.0, 1.0]), r_cut, n_max, l_max)
+    s.beta = w.random_beta(rng, S, P)
+    s.sigma = w.random_sigma(rng, S, P)
+    for sparse in (True, False):
+        assert_parity(oracle, torch, flare, s, nbr_method=0, species_sparse=sparse)
 
 
 def test_paper_basis_7_3_dimension_420(oracle, torch, flare):
@@ -280,3 +311,20 @@ def test_tile_16k_atoms_sampled(oracle, torch, flare):
     cnt_g, idx_g = ctx.neighbors()
     assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
     assert np.abs(f.sum(0)).max() < 1e-9
+
+
+def test_isolated_atoms_in_sparse_mode(oracle, torch, flare):
+    """Atoms without neighbours form an empty (species, mask=0) group: E = V = 0, no forces, no table reads."""
+    rng = np.random.default_rng(51)
+    box = np.diag([40.0, 40, 40]).reshape(9)
+    pos = np.concatenate([rng.uniform(0, 40, (30, 3)), 20 + rng.uniform(-2.5, 2.5, (40, 3))])
+    keep = [0]
+    for i in range(1, len(pos)):
+        if np.min(np.linalg.norm(pos[keep] - pos[i], axis=1)) > 1.0:
+            keep.append(i)
+    pos = pos[keep]
+    types = rng.integers(0, 2, len(keep))
+    s = _mk(pos, types, box, [1, 1, 1], 2, n_max=3, l_max=2, seed=52)
+    ctx, got, want = assert_parity(oracle, torch, flare, s, nbr_method=0, species_sparse=True)
+    cnt, _ = ctx.neighbors()
+    assert (cnt == 0).sum() > 5 and (got[0][cnt == 0] == 0).all() and (got[1][cnt == 0] == 0).all()
