@@ -182,7 +182,8 @@ def run_ours(args):
     want_var = not args.no_variance
     n = s.n_atoms
     ctx = flare.from_system(s, device=local, variance=want_var, timing=True,
-                            chunk_atoms=args.chunk if args.chunk else None)
+                            chunk_atoms=args.chunk if args.chunk else None,
+                            species_sparse=False if args.dense else None)
     ctx.bind(n)
     dt_fs = float(s.meta.get("dt_fs", 0.5))
     pos = torch.as_tensor(s.pos, dtype=torch.float64, device=dev)
@@ -265,7 +266,10 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel: the quadratic-form DMMA GEMM
     P = s.P
-    flops_per_step = float(n) * 2.0 * P * P * (2 if want_var else 1)
+    sparse = bool(ctx.get_option(flare.OPT_SPECIES_SPARSE))
+    groups = [g for g in ctx.groups() if g[0] > 0]
+    flops_per_step = ctx.qform_flops(want_var)  # sum over atoms of 2 P_g^2 per form (P_g = P without sparsity)
+    qf_bytes_per_step = float(sum(r * 8.0 * p * (2 if want_var else 1) + r * 8.0 * p for r, p in groups))
     qf_ms, qf_launches = phases["qform"]
     qf_ms_per_step = qf_ms / args.steps
     achieved = flops_per_step / (qf_ms_per_step * 1e-3) * 1e-12 if qf_ms_per_step > 0 else 0.0
@@ -281,7 +285,9 @@ def run_ours(args):
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
         # dram__bytes_read+write of k_qform per atom row, from the ncu --set full capture in
         # profiles/r01_qform_full.md (1.771 GB for the 205 184-row launch), scaled to one step's rows
-        "traffic": 8630.0 * n if P == 544 else None,
+        "traffic": 8630.0 * n if (P == 544 and not sparse) else None,
+        "algorithmic_bytes": qf_bytes_per_step,
+        "groups_rows_x_components": groups,
         "peak_source": "FP64 DMMA issue peak measured live by flare_measure_fp64_dmma_peak "
                        "(MEASURED_PEAKS.json has no FP64 entry; its sustained bf16 x nominal 45/2250 gives "
                        f"{derived:.1f} TFLOP/s)" if derived else "FP64 DMMA issue peak measured live",
@@ -295,6 +301,7 @@ def run_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "atoms": n, "P": P, "variance": want_var, "dt_fs": dt_fs,
+                   "species_sparse": sparse,
                    "chunk_atoms": ctx.get_option(flare.OPT_CHUNK_ATOMS),
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": "working set (>10 GB of descriptors per step) is far larger than the 126 MB L2; no flush needed"},
@@ -323,6 +330,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-variance", action="store_true")
+    ap.add_argument("--dense", action="store_true", help="switch the species-sparse evaluation (P:L155) off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

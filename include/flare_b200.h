@@ -171,6 +171,13 @@ int flare_get_neighbors(flare_ctx* ctx, int32_t* cnt, int32_t* idx, int32_t stri
 int flare_get_descriptors(flare_ctx* ctx, double* bhat, double* nrm);
 
 /*
+ * Row statistics of the last evaluation's quadratic-form groups (synchronises; HOST outputs):
+ * n_groups, and per group the number of atoms (rows) and of descriptor components it uses
+ * (arrays of at least 64 entries).  The algorithmic flop count of steps a4/a5 is sum rows * 2 comps^2.
+ */
+int flare_get_groups(flare_ctx* ctx, int32_t* n_groups, int64_t* rows, int32_t* comps);
+
+/*
  * Accumulated CUDA-event time (ms) and launch count per phase since the last call
  * (needs FLARE_OPT_TIMING = 1); ms and launches are [FLARE_N_PHASES] host arrays.  Synchronises.
  */

@@ -739,6 +739,24 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
     return FLARE_OK;
 }
 
+int flare_get_groups(flare_ctx* c, int32_t* n_groups, int64_t* rows, int32_t* comps) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->have_grid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    if (!n_groups || !rows || !comps) return fail(c, FLARE_ERR_INVALID_ARG, "bad output arrays");
+    rc = flare_check(c);
+    if (rc) return rc;
+    std::vector<int> start(c->n_groups + 1, 0);
+    if (c->n > 0)
+        FLARE_CUDA(c, cudaMemcpy(start.data(), c->ws.group_start, sizeof(int) * (c->n_groups + 1), cudaMemcpyDeviceToHost));
+    *n_groups = c->n_groups;
+    for (int g = 0; g < c->n_groups; g++) {
+        rows[g] = start[g + 1] - start[g];
+        comps[g] = c->groups[g].P;
+    }
+    return FLARE_OK;
+}
+
 int flare_get_timings(flare_ctx* c, double* ms, int64_t* launches) {
     if (!c || !ms) return FLARE_ERR_INVALID_ARG;
     FLARE_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -29,7 +29,7 @@ EXPORTS = (
     "flare_create", "flare_destroy", "flare_num_descriptors", "flare_set_option", "flare_get_option",
     "flare_workspace_bytes", "flare_bind", "flare_compute", "flare_compute_host", "flare_check",
     "flare_set_state", "flare_set_state_host", "flare_set_forces", "flare_set_forces_host", "flare_step", "flare_get_state", "flare_get_state_host",
-    "flare_get_neighbors", "flare_get_descriptors", "flare_get_timings", "flare_kernel_launches",
+    "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_timings", "flare_kernel_launches",
     "flare_measure_fp64_dmma_peak", "flare_last_error",
 )
 
@@ -74,6 +74,7 @@ def load_library():
     lib.flare_get_state_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.flare_get_neighbors.argtypes = [vp, vp, vp, C.c_int32]
     lib.flare_get_descriptors.argtypes = [vp, vp, vp]
+    lib.flare_get_groups.argtypes = [vp, vp, vp, vp]
     lib.flare_get_timings.argtypes = [vp, vp, vp]
     lib.flare_kernel_launches.argtypes = [vp]
     lib.flare_kernel_launches.restype = i64
@@ -295,6 +296,18 @@ class Flare:
         nrm = np.zeros(n)
         self._check(self._lib.flare_get_descriptors(self._ctx, _hp(bh), _hp(nrm)))
         return bh, nrm
+
+    def groups(self):
+        """[(rows, components)] of the quadratic-form groups of the last evaluation."""
+        n = C.c_int32(0)
+        rows = np.zeros(64, np.int64)
+        comps = np.zeros(64, np.int32)
+        self._check(self._lib.flare_get_groups(self._ctx, C.cast(C.byref(n), C.c_void_p), _hp(rows), _hp(comps)))
+        return [(int(rows[g]), int(comps[g])) for g in range(n.value)]
+
+    def qform_flops(self, variance: bool) -> float:
+        """Algorithmic flops of steps a4 (+ a5): sum over atoms of 2 P_g^2 per form."""
+        return float(sum(r * 2.0 * p * p for r, p in self.groups()) * (2 if variance else 1))
 
     def timings(self):
         ms = np.zeros(len(PHASES))
