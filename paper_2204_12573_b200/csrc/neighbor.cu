@@ -190,6 +190,10 @@ __device__ __forceinline__ int slow_cells(const Grid& g, int d, int c, int out[3
 
 constexpr int kNbrWarps = 8;
 
+// One warp per atom.  The (up to 3 x 3 x 2) contiguous runs of candidate atoms -- one per (slow1, slow0)
+// cell column and fast-dimension range -- are looked up by the first lanes in parallel, laid end to end by a
+// warp scan, and the concatenation is swept 32 candidates at a time, so that every lane tests one candidate
+// per sweep whatever the run lengths are (a sweep per run would leave most lanes idle: a run holds ~15 atoms).
 __global__ void __launch_bounds__(kNbrWarps * 32)
 k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int* __restrict__ cell_start, int mmax,
             int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx, unsigned char* __restrict__ nmask,
@@ -206,37 +210,56 @@ k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int*
     const int na = slow_cells(g, g.slow0, c[g.slow0], ca);
     const int nb = slow_cells(g, g.slow1, c[g.slow1], cb);
     const int nf = fast_ranges(g, c[g.fast], flo, fhi);
+    // run rr = (ib * na + ia) * nf + r: same visiting order as nested loops over (ib, ia, r)
+    const int nr = nb * na * nf;  // <= 18
+    int rs = 0, len = 0;
+    if (lane < nr) {
+        const int r = lane % nf, t = lane / nf;
+        const int ia = t % na, ib = t / na;
+        const int base = ca[ia] * g.stride[g.slow0] + cb[ib] * g.stride[g.slow1];
+        rs = __ldg(cell_start + base + flo[r]);
+        len = __ldg(cell_start + base + fhi[r] + 1) - rs;
+    }
+    int inc = len;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(kFull, inc, o);
+        if (lane >= o) inc += y;
+    }
+    const int total = __shfl_sync(kFull, inc, 31);
+    const int exc = inc - len;  // position of the run's first candidate in the concatenation
     int* row = nbr_idx + (size_t)k * mmax;
     int cnt = 0;
     unsigned mask = 0;
     const double* rc2 = bs.rc2 + me.type * bs.S;
-    for (int ib = 0; ib < nb; ib++)
-        for (int ia = 0; ia < na; ia++) {
-            const int base = ca[ia] * g.stride[g.slow0] + cb[ib] * g.stride[g.slow1];
-            for (int r = 0; r < nf; r++) {
-                const int s = cell_start[base + flo[r]];
-                const int e = cell_start[base + fhi[r] + 1];
-                for (int q0 = s; q0 < e; q0 += 32) {
-                    const int q = q0 + lane;
-                    bool hit = false;
-                    int tj = 0;
-                    if (q < e && q != k) {
-                        const AtomS o = load_atom(atoms + q);
-                        double dx, dy, dz;
-                        displacement(g, me, o, dx, dy, dz);
-                        tj = o.type;
-                        hit = dist2_canonical(dx, dy, dz) < rc2[tj];  // strict (R6)
-                    }
-                    const unsigned b = __ballot_sync(kFull, hit);
-                    if (hit) {
-                        const int slot = cnt + __popc(b & ((1u << lane) - 1u));
-                        if (slot < mmax) row[slot] = q;
-                        mask |= 1u << tj;
-                    }
-                    cnt += __popc(b);
-                }
-            }
+    for (int c0 = 0; c0 < total; c0 += 32) {
+        const int ci = c0 + lane;
+        // last run whose first position is <= ci (empty runs share their successor's position and lose the tie)
+        int pos = 0;
+#pragma unroll
+        for (int st = 16; st > 0; st >>= 1) {
+            const int t = pos + st;
+            const int v = __shfl_sync(kFull, exc, t & 31);
+            if (t < 32 && v <= ci) pos = t;
         }
+        const int q = __shfl_sync(kFull, rs, pos) + (ci - __shfl_sync(kFull, exc, pos));
+        bool hit = false;
+        int tj = 0;
+        if (ci < total && q != k) {
+            const AtomS o = load_atom(atoms + q);
+            double dx, dy, dz;
+            displacement(g, me, o, dx, dy, dz);
+            tj = o.type;
+            hit = dist2_canonical(dx, dy, dz) < rc2[tj];  // strict (R6)
+        }
+        const unsigned b = __ballot_sync(kFull, hit);
+        if (hit) {
+            const int slot = cnt + __popc(b & ((1u << lane) - 1u));
+            if (slot < mmax) row[slot] = q;
+            mask |= 1u << tj;
+        }
+        cnt += __popc(b);
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mask |= __shfl_xor_sync(kFull, mask, o);
     if (lane == 0) {
@@ -246,7 +269,10 @@ k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int*
     }
 }
 
-// rev[k][s] = slot of k in the row of j = nbr_idx[k][s]  (exists because cutoffs are symmetric, R5)
+// rev[k][s] = slot of k in the row of j = nbr_idx[k][s]  (exists because cutoffs are symmetric, R5).
+// Lane s holds neighbour s and its row length; the rows of four neighbours are fetched together (one
+// coalesced 128-byte read each) before any of them is searched, and the found slots are written back as
+// one coalesced byte store per 32 neighbours.
 __global__ void __launch_bounds__(kNbrWarps * 32)
 k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx,
                 unsigned char* __restrict__ rev) {
@@ -254,17 +280,33 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
     const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
     if (k >= n) return;
     const int cnt = nbr_cnt[k];
-    for (int s = 0; s < cnt; s++) {
-        const int j = nbr_idx[(size_t)k * mmax + s];
-        const int cj = nbr_cnt[j];
-        int found = 0;
-        for (int b = 0; b < cj; b += 32) {
-            const int t = b + lane;
-            const bool eq = (t < cj) && (nbr_idx[(size_t)j * mmax + t] == k);
-            const unsigned m = __ballot_sync(kFull, eq);
-            if (m) { found = b + __ffs(m) - 1; break; }
+    for (int base = 0; base < cnt; base += 32) {
+        const int s = base + lane;
+        const int nact = min(32, cnt - base);
+        int j = 0, cj = 0;
+        if (s < cnt) { j = nbr_idx[(size_t)k * mmax + s]; cj = nbr_cnt[j]; }
+        int mine = 0;
+        for (int t0 = 0; t0 < nact; t0 += 4) {
+            int jj[4], cc[4], v[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                jj[u] = __shfl_sync(kFull, j, (t0 + u) & 31);
+                cc[u] = __shfl_sync(kFull, cj, (t0 + u) & 31);  // 0 beyond nact: nothing is read
+                v[u] = (lane < cc[u]) ? nbr_idx[(size_t)jj[u] * mmax + lane] : -1;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                unsigned m = __ballot_sync(kFull, v[u] == k);
+                int found = m ? __ffs(m) - 1 : 0;
+                for (int b = 32; !m && b < cc[u]; b += 32) {  // rows longer than a warp
+                    const int t = b + lane;
+                    m = __ballot_sync(kFull, (t < cc[u]) && (nbr_idx[(size_t)jj[u] * mmax + t] == k));
+                    if (m) found = b + __ffs(m) - 1;
+                }
+                if (lane == t0 + u) mine = found;
+            }
         }
-        if (lane == 0) rev[(size_t)k * mmax + s] = (unsigned char)found;
+        if (s < cnt) rev[(size_t)k * mmax + s] = (unsigned char)mine;
     }
 }
 
@@ -288,18 +330,27 @@ k_group_hist(int n, int S, int sparse, int n_groups, const AtomS* __restrict__ a
     for (int t = threadIdx.x; t < n_groups; t += blockDim.x) hist[(size_t)blockIdx.x * n_groups + t] = h[t];
 }
 
-// one thread per group walks the blocks; then thread 0 lays the groups out one after another
-__global__ void k_group_scan(int n_blocks, int n_groups, int* __restrict__ hist, int* __restrict__ group_start) {
+// one warp per group scans that group's per-block counts (exclusive, in place); then thread 0 lays the groups
+// out one after another
+__global__ void __launch_bounds__(32 * 32)
+k_group_scan(int n_blocks, int n_groups, int* __restrict__ hist, int* __restrict__ group_start) {
     __shared__ int tot[kMaxGroups + 1];
-    int gidx = threadIdx.x;
-    if (gidx < n_groups) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int gidx = w; gidx < n_groups; gidx += 32) {
         int run = 0;
-        for (int b = 0; b < n_blocks; b++) {
-            int v = hist[(size_t)b * n_groups + gidx];
-            hist[(size_t)b * n_groups + gidx] = run;
-            run += v;
+        for (int b0 = 0; b0 < n_blocks; b0 += 32) {
+            const int b = b0 + lane;
+            const int v = (b < n_blocks) ? hist[(size_t)b * n_groups + gidx] : 0;
+            int x = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(kFull, x, o);
+                if (lane >= o) x += y;
+            }
+            if (b < n_blocks) hist[(size_t)b * n_groups + gidx] = run + x - v;
+            run += __shfl_sync(kFull, x, 31);
         }
-        tot[gidx] = run;
+        if (lane == 0) tot[gidx] = run;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -355,7 +406,7 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
     const int ngb = (n + kGroupBlock - 1) / kGroupBlock;
     L.launch(k_group_hist, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
              (const unsigned char*)ws.nmask, ws.group_hist);
-    L.launch(k_group_scan, dim3(1), dim3(kMaxGroups), 0, ngb, n_groups, ws.group_hist, ws.group_start);
+    L.launch(k_group_scan, dim3(1), dim3(32 * 32), 0, ngb, n_groups, ws.group_hist, ws.group_start);
     L.launch(k_group_assign, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
              (const unsigned char*)ws.nmask, (const int*)ws.group_hist, (const int*)ws.group_start, ws.row_of,
              ws.atom_of_row, ws.gid);
