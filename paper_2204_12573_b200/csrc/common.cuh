@@ -47,6 +47,7 @@ struct Basis {
     int Pld;     // padded row length of B^/W rows (multiple of 16)
     double rc[kMaxSpecies * kMaxSpecies];
     double rc2[kMaxSpecies * kMaxSpecies];
+    double irc[kMaxSpecies * kMaxSpecies];  // 1 / r_cut
 };
 
 // ------------------------------------------------------------------ canonical geometry (R6)

@@ -1,24 +1,40 @@
-// descriptor.cu -- steps a2 + a3: per-pair basis, A accumulation, B2 contraction, normalisation
-// (P:L123-129).  One warp per atom:
-//   1. neighbours are spread across lanes for the basis evaluation (sqrt, sincospi, Chebyshev and
-//      Y_lm recurrences); g~_n and Y_lm of up to 32 neighbours are staged in shared memory;
-//   2. A[nu,lm] = sum_j [s_j = s] g~_n(j) Y_lm(j) is a small dense contraction over the neighbours
-//      (an [N_nu x M] . [M x L^2] product); it runs on the FP64 tensor pipe (mma.sync m8n8k4) with
-//      the species selection folded into the A-operand, so no shuffle reduction over the 256+
-//      components and no per-component shared-memory loop is needed;
-//   3. B[nu1<=nu2, l] = sum_m A[nu1,l,m] A[nu2,l,m]: one (nu1,nu2) pair per lane, all l at once, so a
-//      warp writes 32 x (l_max+1) consecutive doubles of the B^ row (fully coalesced); two passes
-//      (norm, then scaled store) recompute the cheap contraction instead of holding B in registers.
+// descriptor.cu -- steps a2 + a3: per-pair basis, A accumulation, B2 contraction.
+// One launch per (chunk, group); a group's atoms share the set of neighbour species, so the
+// whole launch works on the group's Nc = nsp * n_max compact radial channels.
+//
+// A warp owns kDescTA consecutive rows (atoms) and walks over the concatenation of their
+// neighbour lists in passes of 32 pairs, one pair per lane, so that the transcendental work
+// (rsqrt, cospi, Chebyshev and Y_lm recurrences) runs with nearly full lanes although one atom
+// has only 12-18 neighbours:
+//   1. stage: lane p evaluates g~_n and Y_lm of its pair and writes them, pair-contiguous, into
+//      shared memory ([n][pair] and [lm][pair], row stride 36: conflict-free fragment loads);
+//   2. accumulate: for every atom with pairs in the pass, A[cnu,lm] += sum_j [s_j = s] g~_n(j) Y_lm(j)
+//      as an [Nc x M].[M x L^2] product on the FP64 tensor pipe (mma.sync m8n8k4), the species
+//      selection folded into the A-operand;
+//   3. finalize (when the atom's last pair has been consumed): A -> global (for the back-propagation),
+//      B[cnu1 <= cnu2, l] = sum_m A[cnu1,l,m] A[cnu2,l,m] as per-l [Nc x (2l+1)].[(2l+1) x Nc] products on
+//      the tensor pipe, stored straight from the accumulator fragments (the L values of one (cnu1,cnu2)
+//      pair are contiguous), and ||B||.  B is stored UNNORMALISED: d^ = B/||B|| is applied by the
+//      consumers (E = B^T beta B / ||B||^2), which saves a second pass over the row.
 #include "kernels.cuh"
 
 namespace flare {
 
 constexpr int kDescWarps = 4;
+constexpr int kDescTA = 8;  // atoms per warp
+constexpr int kPS = 36;     // pair stride of the staged rows (= 4 mod 16)
 
-__host__ __device__ inline int desc_warp_doubles(int n_max, int L2, int Nv) {
-    // g[32][n_max|1], Y[32][L2|1], A[Nv][L2|1], species[32] (ints, 16 doubles)
-    return 32 * (n_max | 1) + 32 * (L2 | 1) + Nv * (L2 | 1) + 16;
+__host__ __device__ constexpr int pad4mod16(int n) {  // smallest m >= n with m % 16 == 4
+    return ((n + 11) / 16) * 16 + 4;
 }
+
+template <int LMAX, int NMAXP>
+struct DescSmem {
+    static constexpr int L2 = (LMAX + 1) * (LMAX + 1);
+    static constexpr int YR = ((L2 + 7) / 8) * 8;  // Y rows incl. zero padding up to a multiple of 8
+    static constexpr int AS = pad4mod16(YR);       // row stride of A (conflict-free operand loads)
+    __host__ __device__ static int warp_doubles(int Nc8) { return NMAXP * kPS + YR * kPS + Nc8 * AS + 16; }
+};
 
 __device__ __forceinline__ void dmma884_d(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -26,151 +42,222 @@ __device__ __forceinline__ void dmma884_d(double& c0, double& c1, double a, doub
                  : "d"(a), "d"(b));
 }
 
-template <int LMAX>
+template <int LMAX, int NMAXP>
 __global__ void __launch_bounds__(kDescWarps * 32)
-k_descriptor(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
+k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
              const int* __restrict__ nbr_idx, int mmax, const int* __restrict__ atom_of_row,
-             const unsigned char* __restrict__ gid, const GroupDev* __restrict__ groups, int row0, int nrows,
-             double* __restrict__ A_out, double* __restrict__ bh_out, int ld, double* __restrict__ nrm_out,
-             const int* __restrict__ out_map) {
+             const int* __restrict__ group_start, double* __restrict__ A_out, double* __restrict__ b_out, int ld,
+             double* __restrict__ nrm_out) {
+    using SM = DescSmem<LMAX, NMAXP>;
     constexpr int L = LMAX + 1;
     constexpr int L2 = L * L;
-    constexpr int YS = L2 | 1;  // odd row strides: conflict-free column access across rows
-    constexpr int AS = L2 | 1;
-    extern __shared__ double smem[];
+    constexpr int NBY = SM::YR / 8;
+    constexpr int AS = SM::AS;
+    extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int local = blockIdx.x * kDescWarps + warp;
-    if (local >= nrows) return;  // warps are independent: only __syncwarp below
+    // rows of this group inside the chunk
+    const int gs_ = max(group_start[gr.g], gr.row0);
+    const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
+    const int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA;
+    if (r0 >= ge_ - gs_) return;  // warps are independent: only __syncwarp below
+    const int na = min(kDescTA, ge_ - gs_ - r0);
+    const int lrow0 = gs_ - gr.row0 + r0;  // chunk-local row of the warp's first atom
     const int g8 = lane >> 2, t4 = lane & 3;
-    const int GS = bs.n_max | 1;
-    const int Nv = bs.Nv;
-    double* gs = smem + (size_t)warp * desc_warp_doubles(bs.n_max, L2, Nv);
-    double* ys = gs + 32 * GS;
-    double* As = ys + 32 * YS;
-    int* sjs = reinterpret_cast<int*>(As + Nv * AS);
+    const int n_max = bs.n_max;
+    const int Nc = gr.Nc, Nc8 = (Nc + 7) & ~7, nmb = Nc8 >> 3;
+    double* gsm = smem + (size_t)warp * SM::warp_doubles(Nc8);  // [NMAXP][kPS]
+    double* ysm = gsm + NMAXP * kPS;                             // [YR][kPS]
+    double* As = ysm + SM::YR * kPS;                             // [Nc8][AS]
+    int* sjs = reinterpret_cast<int*>(As + Nc8 * AS);            // [32] compact species of the staged pairs
+    for (int c = lane; c < (NMAXP + SM::YR) * kPS + Nc8 * AS; c += 32) gsm[c] = 0.0;
 
-    const int k = atom_of_row[row0 + local];
-    const AtomS me = load_atom(atoms + k);
-    const int cnt = nbr_cnt[k];
-    for (int c = lane; c < Nv * AS; c += 32) As[c] = 0.0;
+    // per-lane atom bookkeeping (lanes 0..na-1), inclusive scan of the neighbour counts
+    int my_k = 0, my_cnt = 0;
+    if (lane < na) {
+        my_k = atom_of_row[gs_ + r0 + lane];
+        my_cnt = nbr_cnt[my_k];
+    }
+    int my_end = my_cnt;
+#pragma unroll
+    for (int o = 1; o < kDescTA; o <<= 1) {
+        const int v = __shfl_up_sync(kFull, my_end, o);
+        if (lane >= o) my_end += v;
+    }
+    const int my_start = my_end - my_cnt;
+    const int T = __shfl_sync(kFull, my_end, kDescTA - 1);
+    __syncwarp();
 
-    for (int base = 0; base < cnt; base += 32) {
-        const int nact = min(32, cnt - base);
-        int sj = -1;
-        if (lane < nact) {
-            const int j = nbr_idx[(size_t)k * mmax + base + lane];
-            const AtomS o = load_atom(atoms + j);
-            double dx, dy, dz;
-            displacement(g, me, o, dx, dy, dz);
-            const double r = sqrt(dx * dx + dy * dy + dz * dz);
-            const double ir = 1.0 / r;
-            sj = o.type;
-            double* gl = gs + lane * GS;
-            radial_basis<false>(bs.n_max, r, bs.rc[me.type * bs.S + sj], [&](int n, double gv, double) { gl[n] = gv; });
-            double* yl = ys + lane * YS;
-            real_ylm<LMAX, false>(yn, dx * ir, dy * ir, dz * ir,
-                                  [&](int lm, double Y, double, double, double) { yl[lm] = Y; });
-        }
-        sjs[lane] = sj;
-        __syncwarp();
-        // A += G^T Y on the tensor pipe.  Fragment roles (m8n8k4): A-operand (row nu = 8mb+g8, col j = k0+t4),
-        // B-operand (row j = k0+t4, col lm = 8nb+g8), C (row nu = 8mb+g8, cols lm = 8nb+2t4, +1).
-        for (int mb = 0; mb * 8 < Nv; mb++) {
-            const int nu = mb * 8 + g8;
-            const int s_nu = (nu < Nv) ? nu / bs.n_max : -2;
-            const int n_nu = nu - s_nu * bs.n_max;
-#pragma unroll 1
-            for (int nb = 0; nb * 8 < L2; nb++) {
-                const int lmb = nb * 8 + g8;
-                double c0 = 0.0, c1 = 0.0;
-                for (int k0 = 0; k0 < nact; k0 += 4) {
-                    const int j = k0 + t4;  // < 32 always; lanes >= nact carry sjs = -1
-                    const double a = (sjs[j] == s_nu) ? gs[j * GS + n_nu] : 0.0;
-                    const double b = (j < nact && lmb < L2) ? ys[j * YS + lmb] : 0.0;
-                    dmma884_d(c0, c1, a, b);
+    int a = 0;
+    for (int p0 = 0;; p0 += 32) {
+        // ---- 1. stage the basis of pairs [p0, p0+32)
+        if (p0 < T) {
+            const int p = p0 + lane;
+            int ai = 0;
+#pragma unroll
+            for (int i = 0; i < kDescTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
+            const int k = __shfl_sync(kFull, my_k, ai);
+            const int s = p - __shfl_sync(kFull, my_start, ai);
+            int sj = -1;
+            if (p < T) {
+                const int j = nbr_idx[(size_t)k * mmax + s];
+                const AtomS me = load_atom(atoms + k);
+                const AtomS o = load_atom(atoms + j);
+                double dx, dy, dz;
+                displacement(g, me, o, dx, dy, dz);
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                const double ir = rsqrt(r2);
+                const double r = r2 * ir;
+                sj = (int)((gr.sidx >> (4 * o.type)) & 15u);
+                const double q = r * bs.irc[me.type * bs.S + o.type];
+                const double x = 2.0 * q - 1.0;
+                const double fc = 0.5 + 0.5 * cospi(q);
+                double t0 = fc, t1 = x * fc;  // T_n(x) f_c
+                const double x2 = 2.0 * x;
+#pragma unroll
+                for (int n = 0; n < NMAXP; n++) {
+                    if (n < n_max) gsm[n * kPS + lane] = t0;
+                    const double t2 = x2 * t1 - t0;
+                    t0 = t1; t1 = t2;
                 }
-                const int lm0 = nb * 8 + 2 * t4;
-                if (nu < Nv) {
-                    if (lm0 < L2) As[nu * AS + lm0] += c0;
-                    if (lm0 + 1 < L2) As[nu * AS + lm0 + 1] += c1;
+                real_ylm<LMAX, false>(yn, dx * ir, dy * ir, dz * ir,
+                                      [&](int lm, double Y, double, double, double) { ysm[lm * kPS + lane] = Y; });
+            }
+            sjs[lane] = sj;
+        }
+        __syncwarp();
+        // ---- 2./3. consume: every atom with pairs in this pass, in order
+        while (a < na) {
+            const int a_start = __shfl_sync(kFull, my_start, a);
+            const int a_end = __shfl_sync(kFull, my_end, a);
+            const int s0 = max(a_start, p0) - p0, s1 = min(a_end, p0 + 32) - p0;
+            if (s1 > s0) {
+                // A += G^T Y.  Fragment roles (m8n8k4): A-operand (row cnu = 8mb+g8, col j = k0+t4),
+                // B-operand (row j = k0+t4, col lm = 8nb+g8), C (row cnu = 8mb+g8, cols lm = 8nb+2t4, +1).
+                for (int mb = 0; mb < nmb; mb++) {
+                    const int cnu = mb * 8 + g8;
+                    const int s_nu = (cnu < Nc) ? cnu / n_max : -2;
+                    const double* grow = gsm + (cnu < Nc ? cnu - s_nu * n_max : 0) * kPS;
+                    double acc[NBY][2];
+#pragma unroll
+                    for (int nb = 0; nb < NBY; nb++) { acc[nb][0] = 0.0; acc[nb][1] = 0.0; }
+                    for (int k0 = s0 & ~3; k0 < s1; k0 += 4) {
+                        const int j = k0 + t4;
+                        const bool on = (j >= s0) && (j < s1) && (sjs[j] == s_nu);
+                        const double av = on ? grow[j] : 0.0;
+#pragma unroll
+                        for (int nb = 0; nb < NBY; nb++)
+                            dmma884_d(acc[nb][0], acc[nb][1], av, ysm[(nb * 8 + g8) * kPS + j]);
+                    }
+                    double* arow = As + cnu * AS + 2 * t4;
+#pragma unroll
+                    for (int nb = 0; nb < NBY; nb++) {
+                        double2* dst = reinterpret_cast<double2*>(arow + nb * 8);
+                        double2 v = *dst;
+                        v.x += acc[nb][0]; v.y += acc[nb][1];
+                        *dst = v;
+                    }
+                }
+                __syncwarp();
+            }
+            if (a_end > p0 + 32) break;  // the atom continues in the next pass
+            // ---- finalize atom a
+            const int lrow = lrow0 + a;
+            if (A_out) {
+                double* arow = A_out + (size_t)lrow * bs.NvL2;
+                for (int c = lane; c < Nc * L2; c += 32) {
+                    const int nu = c / L2;
+                    arow[c] = As[nu * AS + (c - nu * L2)];
                 }
             }
+            double* brow = b_out + (size_t)lrow * ld;
+            double n2 = 0.0;
+            for (int mb = 0; mb < nmb; mb++) {
+                const int nu1 = mb * 8 + g8;
+                const double* a1 = As + nu1 * AS + t4;
+                for (int nb = mb; nb < nmb; nb++) {
+                    const double* a2 = As + (nb * 8 + g8) * AS + t4;
+                    double acc[L][2];
+#pragma unroll
+                    for (int l = 0; l < L; l++) {
+                        acc[l][0] = 0.0; acc[l][1] = 0.0;
+#pragma unroll
+                        for (int ks = 0; ks < (2 * l + 1 + 3) / 4; ks++) {
+                            const bool ok = 4 * ks + t4 < 2 * l + 1;
+                            const double av = ok ? a1[l * l + 4 * ks] : 0.0;
+                            const double bv = ok ? a2[l * l + 4 * ks] : 0.0;
+                            dmma884_d(acc[l][0], acc[l][1], av, bv);
+                        }
+                    }
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        const int nu2 = nb * 8 + 2 * t4 + e;
+                        if (nu1 <= nu2 && nu2 < Nc) {
+                            // triangular enumeration over the compact channels (R4 order restricted to the group)
+                            const int q = nu1 * Nc - (nu1 * (nu1 - 1)) / 2 + (nu2 - nu1);
+                            double* dst = brow + (size_t)q * L;
+#pragma unroll
+                            for (int l = 0; l < L; l++) n2 = fma(acc[l][e], acc[l][e], n2);
+                            if constexpr (L % 2 == 0) {
+#pragma unroll
+                                for (int l = 0; l < L; l += 2)
+                                    *reinterpret_cast<double2*>(dst + l) = make_double2(acc[l][e], acc[l + 1][e]);
+                            } else {
+#pragma unroll
+                                for (int l = 0; l < L; l++) dst[l] = acc[l][e];
+                            }
+                        }
+                    }
+                }
+            }
+            n2 = warp_sum(n2);
+            for (int p = gr.P + lane; p < gr.K; p += 32) brow[p] = 0.0;  // zero padding up to K
+            if (lane == 0) nrm_out[lrow] = sqrt(n2);                     // no neighbours: B = 0, ||B|| = 0 (R8)
+            __syncwarp();
+            for (int c = lane; c < Nc8 * AS; c += 32) As[c] = 0.0;
+            __syncwarp();
+            a++;
         }
         __syncwarp();
+        if (a >= na) break;
     }
-
-    if (A_out) {
-        double* arow = A_out + (size_t)local * bs.NvL2;
-        for (int c = lane; c < bs.NvL2; c += 32) {
-            const int nu = c / L2;
-            arow[c] = As[nu * AS + (c - nu * L2)];
-        }
-    }
-
-    // B2 contraction, one (nu1,nu2) pair per lane, all l at once.
-    const GroupDev gd = groups[gid[k]];
-    const int npairs = gd.P / L;
-    double n2 = 0.0;
-    for (int q = lane; q < npairs; q += 32) {
-        const int t = __ldg(gd.table + q);
-        const double* a1 = As + (t & 255) * AS;
-        const double* a2 = As + (t >> 8) * AS;
-#pragma unroll
-        for (int l = 0; l < L; l++) {
-            double b = 0.0;
-#pragma unroll
-            for (int i = l * l; i < (l + 1) * (l + 1); i++) b = fma(a1[i], a2[i], b);
-            n2 = fma(b, b, n2);
-        }
-    }
-    n2 = warp_sum(n2);
-    const double nrm = sqrt(n2);
-    const double inv = (nrm > 0.0) ? 1.0 / nrm : 0.0;  // empty neighbourhood: B^ = 0 (R8)
-    const int orow = out_map ? out_map[k] : local;
-    double* brow = bh_out + (size_t)orow * ld;
-    for (int q = lane; q < npairs; q += 32) {
-        const int t = __ldg(gd.table + q);
-        const double* a1 = As + (t & 255) * AS;
-        const double* a2 = As + (t >> 8) * AS;
-#pragma unroll
-        for (int l = 0; l < L; l++) {
-            double b = 0.0;
-#pragma unroll
-            for (int i = l * l; i < (l + 1) * (l + 1); i++) b = fma(a1[i], a2[i], b);
-            brow[q * L + l] = b * inv;
-        }
-    }
-    for (int p = gd.P + lane; p < min(gd.K, ld); p += 32) brow[p] = 0.0;  // zero padding up to K
-    if (lane == 0) nrm_out[orow] = nrm;
 }
 
-template <int LMAX>
+template <int LMAX, int NMAXP>
 static void launch_descriptor(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
-                              int mmax, const GroupDev* groups, int row0, int nrows, double* bh_out, int ld,
-                              double* nrm_out, const int* out_map, bool write_A) {
-    constexpr int L2 = (LMAX + 1) * (LMAX + 1);
-    const size_t smem = sizeof(double) * kDescWarps * (size_t)desc_warp_doubles(bs.n_max, L2, bs.Nv);
+                              int mmax, const GroupRun& gr, double* bh_out, int ld, double* nrm_out, bool write_A) {
+    using SM = DescSmem<LMAX, NMAXP>;
+    const int Nc8 = (gr.Nc + 7) & ~7;
+    const size_t smem = sizeof(double) * kDescWarps * (size_t)SM::warp_doubles(Nc8);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(k_descriptor<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_descriptor<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    L.launch(k_descriptor<LMAX>, dim3((nrows + kDescWarps - 1) / kDescWarps), dim3(kDescWarps * 32), smem, g, bs, yn,
-             (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax, (const int*)ws.atom_of_row,
-             (const unsigned char*)ws.gid, groups, row0, nrows, write_A ? ws.A : (double*)nullptr, bh_out, ld, nrm_out,
-             out_map);
+    const int per_cta = kDescWarps * kDescTA;
+    L.launch(k_descriptor<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(kDescWarps * 32), smem, g, bs, yn,
+             gr, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
+             (const int*)ws.atom_of_row, (const int*)ws.group_start, write_A ? ws.A : (double*)nullptr, bh_out, ld,
+             nrm_out);
 }
 
 void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
-                     const GroupDev* groups, int row0, int nrows, double* bh_out, int ld, double* nrm_out,
-                     const int* out_map, bool write_A) {
+                     const GroupDesc* groups, int n_groups, int row0, int nrows, double* bh_out, int ld,
+                     double* nrm_out, bool write_A) {
     if (nrows <= 0) return;
-    switch (bs.l_max) {
-#define FLARE_CASE(LM) \
-    case LM: launch_descriptor<LM>(L, g, bs, yn, ws, mmax, groups, row0, nrows, bh_out, ld, nrm_out, out_map, write_A); break;
-        FLARE_CASE(0) FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6)
+    for (int gi = 0; gi < n_groups; gi++) {
+        if (groups[gi].P == 0) continue;  // no neighbours: no descriptor (R8); nothing downstream reads these rows
+        const GroupRun gr = make_group_run(groups[gi], gi, row0, nrows);
+#define FLARE_CASE(LM)                                                                                   \
+    case LM:                                                                                             \
+        if (bs.n_max <= 8) launch_descriptor<LM, 8>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A);       \
+        else if (bs.n_max <= 12) launch_descriptor<LM, 12>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A); \
+        else launch_descriptor<LM, 16>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A);                    \
+        break;
+        switch (bs.l_max) {
+            FLARE_CASE(0) FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6)
+            default: break;
+        }
 #undef FLARE_CASE
-        default: break;
     }
 }
 

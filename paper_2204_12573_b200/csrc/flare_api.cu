@@ -188,6 +188,15 @@ int build_groups(flare_ctx* c, const double* beta, const double* sigma, int spar
             }
         GroupDesc& gd = set.groups[gi];
         gd.P = (int)comp.size();
+        gd.mask = mask;
+        gd.sidx = 0;
+        for (int sp = 0, rank = 0; sp < kMaxSpecies; sp++) {
+            const bool in = sp < S && ((mask >> sp) & 1u);
+            gd.sidx |= (unsigned)(in ? rank : 15) << (4 * sp);
+            if (in) rank++;
+            gd.nsp = rank;
+        }
+        gd.Nc = gd.nsp * bs.n_max;
         set.comps[gi] = comp;
         if (gd.P == 0) { gdev[gi] = GroupDev{0, 0, 0, 0, nullptr, nullptr}; continue; }
         gd.K = round_up(gd.P, 16);
@@ -339,8 +348,8 @@ int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, d
         const int nrows = std::min(c->chunk_cap, n - row0);
         {
             PhaseScope ps(c, FLARE_PHASE_DESCRIPTOR);
-            run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ws.Bh, c->ld,
-                            c->ws.nrm, nullptr, true);
+            run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->groups.data(), c->n_groups, row0, nrows,
+                            c->ws.Bh, c->ld, c->ws.nrm, true);
         }
         {
             PhaseScope ps(c, FLARE_PHASE_QFORM);
@@ -348,8 +357,8 @@ int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, d
         }
         {
             PhaseScope ps(c, FLARE_PHASE_BACKPROP);
-            run_backprop(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ld, c->chunk_cap,
-                         c->max_ntn, want_var);
+            run_backprop(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->groups.data(), c->n_groups, row0, nrows, c->ld,
+                         c->chunk_cap, c->max_ntn, want_var);
         }
     }
     {
@@ -402,7 +411,7 @@ int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_m
     bs.Nv = n_species * n_max;
     bs.NvL2 = bs.Nv * bs.L2;
     bs.P = bs.Nv * (bs.Nv + 1) / 2 * (l_max + 1);
-    for (int i = 0; i < n_species * n_species; i++) { bs.rc[i] = r_cut[i]; bs.rc2[i] = r_cut[i] * r_cut[i]; }
+    for (int i = 0; i < n_species * n_species; i++) { bs.rc[i] = r_cut[i]; bs.rc2[i] = r_cut[i] * r_cut[i]; bs.irc[i] = 1.0 / r_cut[i]; }
     c->mass.assign(mass_amu, mass_amu + n_species);
     c->has_sigma = sigma != nullptr;
     // K_lm sqrt(2 - delta_m0)
@@ -718,8 +727,8 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
     std::vector<double> hb, hn;
     for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
         const int nrows = std::min(c->chunk_cap, n - row0);
-        run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->d_groups, row0, nrows, c->ws.Bh, c->ld, c->ws.nrm,
-                        nullptr, false);
+        run_descriptors(L, c->grid, c->bs, c->yn, c->ws, c->mmax, c->groups.data(), c->n_groups, row0, nrows, c->ws.Bh,
+                        c->ld, c->ws.nrm, false);
         if (L.err != cudaSuccess) return cuda_fail(c, L.err, "descriptor launch");
         hb.resize((size_t)nrows * c->ld);
         hn.resize(nrows);
@@ -732,8 +741,10 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
             const std::vector<int>& comp = comps[h_gid[k]];  // compacted -> dense component (identity in dense mode)
             double* dst = bhat + (size_t)i * P;
             for (int p = 0; p < P; p++) dst[p] = 0.0;
-            for (size_t q = 0; q < comp.size(); q++) dst[comp[q]] = hb[(size_t)r * c->ld + q];
-            nrm[i] = hn[r];
+            // rows hold the unnormalised B; atoms without neighbours (empty group) have no row content at all (R8)
+            const double inv = (!comp.empty() && hn[r] > 0.0) ? 1.0 / hn[r] : 0.0;
+            for (size_t q = 0; q < comp.size(); q++) dst[comp[q]] = hb[(size_t)r * c->ld + q] * inv;
+            nrm[i] = comp.empty() ? 0.0 : hn[r];
         }
     }
     return FLARE_OK;

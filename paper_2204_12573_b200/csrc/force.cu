@@ -15,11 +15,19 @@
 namespace flare {
 
 constexpr int kBpWarps = 4;
+constexpr int kBpMaxTA = 8;  // atoms per warp (upper bound; the launch picks ta <= 8 from the shared-memory budget)
 
-__host__ __device__ inline int bp_warp_doubles(int S, int Nv, int L2, int nmaxp, int ld) {
-    // A[Nv][L2|1], c[ld], G^T[S][L2][nmaxp]
-    return (Nv * (L2 | 1) + ld + S * L2 * nmaxp + 1) & ~1;  // even: keeps every warp's G^T 16-byte aligned
-}
+__host__ __device__ constexpr int bp_pad4mod16(int n) { return ((n + 11) / 16) * 16 + 4; }
+
+template <int LMAX, int NMAXP>
+struct BpSmem {
+    static constexpr int L2 = (LMAX + 1) * (LMAX + 1);
+    static constexpr int AS = bp_pad4mod16(L2);    // row stride of the staged A (conflict-free operand loads)
+    static constexpr int GB = L2 * NMAXP + 2;      // G^T block of one (atom, species): [L2][NMAXP] + bank shift
+    __host__ __device__ static int warp_doubles(int ta, int nsp, int Nc8, int K) {
+        return (ta * nsp * GB + Nc8 * AS + K + 1) & ~1;  // even: every warp's region stays 16-byte aligned
+    }
+};
 
 __device__ __forceinline__ void dmma884_f(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -29,13 +37,13 @@ __device__ __forceinline__ void dmma884_f(double& c0, double& c1, double a, doub
 
 // g[n] = T_n(x) f_c(r), dg[n] = d g[n]/dr for n < n_max, zero above; fully unrolled so that g/dg stay in registers
 template <int NMAXP>
-__device__ __forceinline__ void radial_fixed(int n_max, double r, double rc, double (&gv)[NMAXP], double (&dgv)[NMAXP]) {
-    const double inv_rc = 1.0 / rc;
+__device__ __forceinline__ void radial_fixed(int n_max, double r, double inv_rc, double (&gv)[NMAXP],
+                                             double (&dgv)[NMAXP]) {
     const double q = r * inv_rc;
     const double x = 2.0 * q - 1.0;
     double sn, cs;
     sincospi(q, &sn, &cs);
-    const double fc = 0.5 * (1.0 + cs);
+    const double fc = 0.5 + 0.5 * cs;
     const double dfc = -0.5 * kPi * inv_rc * sn;
     const double dxdr = 2.0 * inv_rc;
     double t0 = 1.0, t1 = x, u0 = 0.0, u1 = 1.0;
@@ -51,116 +59,153 @@ __device__ __forceinline__ void radial_fixed(int n_max, double r, double rc, dou
     }
 }
 
+// One launch per (chunk, group).  A warp owns `ta` consecutive rows: phase 1 forms E, V, c = dE/dB and
+// G = dE/dA of each of its atoms (G on the tensor pipe), phase 2 walks over the concatenated neighbour
+// lists of those atoms, one pair per lane, so that the basis gradients run with nearly full lanes.
 template <int LMAX, int NMAXP>
 __global__ void __launch_bounds__(kBpWarps * 32)
-k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
-           const int* __restrict__ nbr_idx, int mmax, const int* __restrict__ atom_of_row,
-           const unsigned char* __restrict__ gid, const GroupDev* __restrict__ groups, int row0, int nrows,
-           const double* __restrict__ A_in, const double* __restrict__ Bh, const double* __restrict__ W,
-           const double* __restrict__ nrm_in, const double* __restrict__ part, int ld, int chunk_cap, int max_ntn,
-           int want_variance, double* __restrict__ pairf, double* __restrict__ e_s, double* __restrict__ v_s) {
+k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restrict__ atoms,
+           const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx, int mmax,
+           const int* __restrict__ atom_of_row, const int* __restrict__ group_start, const double* __restrict__ A_in,
+           const double* __restrict__ Braw, const double* __restrict__ W, const double* __restrict__ nrm_in,
+           const double* __restrict__ part, int ld, int chunk_cap, int max_ntn, int want_variance,
+           double* __restrict__ pairf, double* __restrict__ e_s, double* __restrict__ v_s) {
+    using SM = BpSmem<LMAX, NMAXP>;
     constexpr int L = LMAX + 1;
     constexpr int L2 = L * L;
-    constexpr int AS = L2 | 1;
+    constexpr int AS = SM::AS;
+    constexpr int GB = SM::GB;
     constexpr int NBL = (2 * LMAX + 1 + 7) / 8;  // n8 blocks needed for the widest m range
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int local = blockIdx.x * kBpWarps + warp;
-    if (local >= nrows) return;
+    const int gs_ = max(group_start[gr.g], gr.row0);
+    const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
+    const int r0 = (blockIdx.x * kBpWarps + warp) * ta;
+    if (r0 >= ge_ - gs_) return;  // warps are independent: only __syncwarp below
+    const int na = min(ta, ge_ - gs_ - r0);
+    const int lrow0 = gs_ - gr.row0 + r0;
     const int g8 = lane >> 2, t4 = lane & 3;
-    const int Nv = bs.Nv;
-    double* Gt = smem + (size_t)warp * bp_warp_doubles(bs.S, Nv, L2, NMAXP, ld);  // [S][L2][NMAXP], 16-byte aligned
-    double* As = Gt + bs.S * L2 * NMAXP;
-    double* cs = As + Nv * AS;
+    const int n_max = bs.n_max;
+    const int Nc = gr.Nc, Nc8 = (Nc + 7) & ~7, nmb = Nc8 >> 3;
+    double* Gt = smem + (size_t)warp * SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);  // [ta][nsp][GB]
+    double* As = Gt + ta * gr.nsp * GB;                                           // [Nc8][AS]
+    double* cs = As + Nc8 * AS;                                                   // [K]
+    for (int c = lane; c < ta * gr.nsp * GB + Nc8 * AS; c += 32) Gt[c] = 0.0;  // G^T (n >= n_max stays 0) and A
 
-    const int k = atom_of_row[row0 + local];
-    const GroupDev gd = groups[gid[k]];
-
-    // ---- E, V from the tile partials (fixed order => deterministic)
-    double E = 0.0, V = 0.0;
-    for (int t = 0; t < gd.ntn; t++) E += part[(size_t)t * chunk_cap + local];
-    if (want_variance)
-        for (int t = 0; t < gd.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + local];
-    const double nrm = nrm_in[local];
-    const double two_inv = (nrm > 0.0) ? 2.0 / nrm : 0.0;
-    if (lane == 0) { e_s[k] = E; v_s[k] = V; }
-    if (gd.P == 0) return;  // no neighbours (R8): E = V = 0 and no pair forces; the group has no tables
-
-    // ---- stage A, zero G^T, stage c = dE/dB with the diagonal pairs pre-doubled (the 1 + delta factor)
-    const double* arow = A_in + (size_t)local * bs.NvL2;
-    for (int c = lane; c < bs.NvL2; c += 32) {
-        const int nu = c / L2;
-        As[nu * AS + (c - nu * L2)] = arow[c];
+    int my_k = 0, my_cnt = 0;
+    if (lane < na) {
+        my_k = atom_of_row[gs_ + r0 + lane];
+        my_cnt = nbr_cnt[my_k];
     }
-    for (int c = lane; c < bs.S * L2 * NMAXP; c += 32) Gt[c] = 0.0;
-    const double* wrow = W + (size_t)local * ld;
-    const double* brow = Bh + (size_t)local * ld;
-    for (int p = lane; p < gd.P; p += 32) {
-        const int t = __ldg(gd.table + p / L);
-        const double dbl = ((t & 255) == (t >> 8)) ? 2.0 : 1.0;
-        cs[p] = dbl * two_inv * (wrow[p] - E * brow[p]);
+    int my_end = my_cnt;
+#pragma unroll
+    for (int o = 1; o < kBpMaxTA; o <<= 1) {
+        const int v = __shfl_up_sync(kFull, my_end, o);
+        if (lane >= o) my_end += v;
     }
+    const int my_start = my_end - my_cnt;
+    const int T = __shfl_sync(kFull, my_end, kBpMaxTA - 1);
     __syncwarp();
 
-    // ---- G[nu1, (l,m)] = sum_nu2 C_l[nu1,nu2] A[nu2,(l,m)] with C_l[nu1,nu2] = c[q(nu1,nu2) L + l]: per l a small
-    // symmetric-matrix product on the tensor pipe.  A-operand (row nu1 = 8mb+g8, col nu2 = k0+t4),
-    // B-operand (row nu2 = k0+t4, col m = 8nb+g8), C (row nu1, cols m = 8nb+2t4, +1).
-    for (int mb = 0; mb * 8 < Nv; mb++) {
-        const int nu1 = mb * 8 + g8;
-        double acc[L][NBL][2];
-#pragma unroll
-        for (int l = 0; l < L; l++)
-#pragma unroll
-            for (int nb = 0; nb < NBL; nb++) { acc[l][nb][0] = 0.0; acc[l][nb][1] = 0.0; }
-        for (int k0 = 0; k0 < Nv; k0 += 4) {
-            const int nu2 = k0 + t4;
-            const bool in = nu1 < Nv && nu2 < Nv;
-            const int q = in ? __ldg(gd.lut + nu1 * Nv + nu2) : -1;
-            const double* a2 = As + (nu2 < Nv ? nu2 : 0) * AS;
-#pragma unroll
-            for (int l = 0; l < L; l++) {
-                const double a = (q >= 0) ? cs[q * L + l] : 0.0;
-#pragma unroll
-                for (int nb = 0; nb < NBL; nb++) {
-                    if (nb * 8 < 2 * l + 1) {
-                        const int m = nb * 8 + g8;
-                        const double b = (nu2 < Nv && m < 2 * l + 1) ? a2[l * l + m] : 0.0;
-                        dmma884_f(acc[l][nb][0], acc[l][nb][1], a, b);
-                    }
-                }
-            }
+    // ---------------- phase 1: per atom E, V, c, G
+    for (int a = 0; a < na; a++) {
+        const int k = __shfl_sync(kFull, my_k, a);
+        const int lrow = lrow0 + a;
+        // E, V from the tile partials (fixed order => deterministic); the rows hold the unnormalised B,
+        // so E = B^T beta B / ||B||^2 and c = dE/dB = (2/||B||^2)(W - E B) with W = beta B   (R10, R11)
+        double E = 0.0, V = 0.0;
+        for (int t = 0; t < gr.ntn; t++) E += part[(size_t)t * chunk_cap + lrow];
+        if (want_variance)
+            for (int t = 0; t < gr.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + lrow];
+        const double nrm = (gr.P > 0) ? nrm_in[lrow] : 0.0;
+        const double inv2 = (nrm > 0.0) ? 1.0 / (nrm * nrm) : 0.0;  // no neighbours: E = V = 0 (R8)
+        E *= inv2;
+        V *= inv2;
+        if (lane == 0) { e_s[k] = E; v_s[k] = V; }
+        if (gr.P == 0) continue;
+
+        const double* arow = A_in + (size_t)lrow * bs.NvL2;
+        for (int c = lane; c < Nc * L2; c += 32) {
+            const int nu = c / L2;
+            As[nu * AS + (c - nu * L2)] = arow[c];
         }
-        if (nu1 < Nv) {
-            const int s1 = nu1 / bs.n_max, n1 = nu1 - s1 * bs.n_max;
-            double* gt = Gt + (size_t)s1 * L2 * NMAXP + n1;
+        const double* wrow = W + (size_t)lrow * ld;
+        const double* brow = Braw + (size_t)lrow * ld;
+        const double two_inv2 = 2.0 * inv2;
+        for (int p = lane; p < gr.P; p += 32) {
+            const int t = __ldg(gr.table + p / L);
+            const double dbl = ((t & 255) == (t >> 8)) ? 2.0 : 1.0;  // the (1 + delta) factor of the diagonal pairs
+            cs[p] = dbl * two_inv2 * (wrow[p] - E * brow[p]);
+        }
+        __syncwarp();
+
+        // G[cnu1, (l,m)] = sum_cnu2 C_l[cnu1,cnu2] A[cnu2,(l,m)], C_l[cnu1,cnu2] = c[q(cnu1,cnu2) L + l]: per l a small
+        // symmetric-matrix product on the tensor pipe.  A-operand (row cnu1 = 8mb+g8, col cnu2 = k0+t4),
+        // B-operand (row cnu2 = k0+t4, col m = 8nb+g8), C (row cnu1, cols m = 8nb+2t4, +1).
+        double* Gta = Gt + (size_t)a * gr.nsp * GB;
+        for (int mb = 0; mb < nmb; mb++) {
+            const int nu1 = mb * 8 + g8;
+            double acc[L][NBL][2];
 #pragma unroll
             for (int l = 0; l < L; l++)
 #pragma unroll
-                for (int nb = 0; nb < NBL; nb++) {
-                    const int m = nb * 8 + 2 * t4;
-                    if (m < 2 * l + 1) gt[(l * l + m) * NMAXP] = acc[l][nb][0];
-                    if (m + 1 < 2 * l + 1) gt[(l * l + m + 1) * NMAXP] = acc[l][nb][1];
+                for (int nb = 0; nb < NBL; nb++) { acc[l][nb][0] = 0.0; acc[l][nb][1] = 0.0; }
+            for (int k0 = 0; k0 < Nc8; k0 += 4) {
+                const int nu2 = k0 + t4;
+                const bool in = nu1 < Nc && nu2 < Nc;
+                const int lo = min(nu1, nu2), hi = max(nu1, nu2);
+                const double* cq = cs + (in ? (lo * Nc - (lo * (lo - 1)) / 2 + (hi - lo)) * L : 0);
+                const double* a2 = As + nu2 * AS + g8;
+#pragma unroll
+                for (int l = 0; l < L; l++) {
+                    const double av = in ? cq[l] : 0.0;
+#pragma unroll
+                    for (int nb = 0; nb < NBL; nb++) {
+                        if (nb * 8 < 2 * l + 1) {
+                            const double bv = (nb * 8 + g8 < 2 * l + 1) ? a2[l * l + nb * 8] : 0.0;
+                            dmma884_f(acc[l][nb][0], acc[l][nb][1], av, bv);
+                        }
+                    }
                 }
+            }
+            if (nu1 < Nc) {
+                const int s1 = nu1 / n_max, n1 = nu1 - s1 * n_max;
+                double* gt = Gta + (size_t)s1 * GB + n1;
+#pragma unroll
+                for (int l = 0; l < L; l++)
+#pragma unroll
+                    for (int nb = 0; nb < NBL; nb++) {
+                        const int m = nb * 8 + 2 * t4;
+                        if (m < 2 * l + 1) gt[(l * l + m) * NMAXP] = acc[l][nb][0];
+                        if (m + 1 < 2 * l + 1) gt[(l * l + m + 1) * NMAXP] = acc[l][nb][1];
+                    }
+            }
         }
+        __syncwarp();
     }
-    __syncwarp();
 
-    // ---- per-pair forces f_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj): lanes over neighbours
-    const AtomS me = load_atom(atoms + k);
-    const int cnt = nbr_cnt[k];
-    for (int base = 0; base < cnt; base += 32) {
-        const int s = base + lane;
-        if (s < cnt) {
+    // ---------------- phase 2: per-pair forces f_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj), one pair per lane
+    for (int p0 = 0; p0 < T; p0 += 32) {
+        const int p = p0 + lane;
+        int ai = 0;
+#pragma unroll
+        for (int i = 0; i < kBpMaxTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
+        const int k = __shfl_sync(kFull, my_k, ai);
+        const int s = p - __shfl_sync(kFull, my_start, ai);
+        if (p < T) {
             const int j = nbr_idx[(size_t)k * mmax + s];
+            const AtomS me = load_atom(atoms + k);
             const AtomS o = load_atom(atoms + j);
             double dx, dy, dz;
             displacement(g, me, o, dx, dy, dz);
-            const double r = sqrt(dx * dx + dy * dy + dz * dz);
-            const double ir = 1.0 / r;
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            const double ir = rsqrt(r2);
+            const double r = r2 * ir;
             const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-            double gr[NMAXP], dgr[NMAXP];
-            radial_fixed<NMAXP>(bs.n_max, r, bs.rc[me.type * bs.S + o.type], gr, dgr);
-            const double* Gj = Gt + (size_t)o.type * L2 * NMAXP;
+            double gr_[NMAXP], dgr[NMAXP];
+            radial_fixed<NMAXP>(n_max, r, bs.irc[me.type * bs.S + o.type], gr_, dgr);
+            const int sj = (int)((gr.sidx >> (4 * o.type)) & 15u);
+            const double* Gj = Gt + (size_t)(ai * gr.nsp + sj) * GB;
             double srad = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
             real_ylm<LMAX, true>(yn, ux, uy, uz, [&](int lm, double Y, double gx, double gy, double gz) {
                 const double2* gp = reinterpret_cast<const double2*>(Gj + lm * NMAXP);
@@ -170,8 +215,8 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
                     const double2 Gv = gp[n2];
                     hr = fma(Gv.x, dgr[2 * n2], hr);
                     hr = fma(Gv.y, dgr[2 * n2 + 1], hr);
-                    hg = fma(Gv.x, gr[2 * n2], hg);
-                    hg = fma(Gv.y, gr[2 * n2 + 1], hg);
+                    hg = fma(Gv.x, gr_[2 * n2], hg);
+                    hg = fma(Gv.y, gr_[2 * n2 + 1], hg);
                 }
                 srad = fma(hr, Y, srad);
                 vx = fma(hg, gx, vx);
@@ -190,38 +235,48 @@ k_backprop(Grid g, Basis bs, YNorm yn, const AtomS* __restrict__ atoms, const in
 
 template <int LMAX, int NMAXP>
 static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
-                            int mmax, const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
-                            bool want_variance) {
-    constexpr int L2 = (LMAX + 1) * (LMAX + 1);
-    const size_t smem = sizeof(double) * kBpWarps * (size_t)bp_warp_doubles(bs.S, bs.Nv, L2, NMAXP, ld);
+                            int mmax, const GroupRun& gr, int ld, int chunk_cap, int max_ntn, bool want_variance) {
+    using SM = BpSmem<LMAX, NMAXP>;
+    const int Nc8 = (gr.Nc + 7) & ~7;
+    // atoms per warp: as many as keep a warp's shared memory near 14 KB (4 CTAs per SM), at least 1, at most 8
+    int ta = kBpMaxTA;
+    if (gr.nsp > 0) {
+        const int budget = 1792 - (Nc8 * SM::AS + gr.K);
+        ta = budget / (gr.nsp * SM::GB);
+        ta = ta < 1 ? 1 : (ta > kBpMaxTA ? kBpMaxTA : ta);
+    }
+    const size_t smem = sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         cudaFuncSetAttribute(k_backprop<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    L.launch(k_backprop<LMAX, NMAXP>, dim3((nrows + kBpWarps - 1) / kBpWarps), dim3(kBpWarps * 32), smem, g, bs, yn,
-             (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
-             (const int*)ws.atom_of_row, (const unsigned char*)ws.gid, groups, row0, nrows, (const double*)ws.A,
-             (const double*)ws.Bh, (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap,
-             max_ntn, want_variance ? 1 : 0, ws.pairf, ws.e_s, ws.v_s);
+    const int per_cta = kBpWarps * ta;
+    L.launch(k_backprop<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(kBpWarps * 32), smem, g, bs, yn, gr,
+             ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
+             (const int*)ws.atom_of_row, (const int*)ws.group_start, (const double*)ws.A, (const double*)ws.Bh,
+             (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap, max_ntn,
+             want_variance ? 1 : 0, ws.pairf, ws.e_s, ws.v_s);
 }
 
 void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
-                  const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
+                  const GroupDesc* groups, int n_groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
                   bool want_variance) {
     if (nrows <= 0) return;
-#define FLARE_CASE(LM)                                                                                                \
-    case LM:                                                                                                          \
-        if (bs.n_max <= 8)                                                                                            \
-            launch_backprop<LM, 8>(L, g, bs, yn, ws, mmax, groups, row0, nrows, ld, chunk_cap, max_ntn, want_variance); \
-        else                                                                                                          \
-            launch_backprop<LM, 16>(L, g, bs, yn, ws, mmax, groups, row0, nrows, ld, chunk_cap, max_ntn, want_variance); \
+    for (int gi = 0; gi < n_groups; gi++) {
+        const GroupRun gr = make_group_run(groups[gi], gi, row0, nrows);
+#define FLARE_CASE(LM)                                                                                        \
+    case LM:                                                                                                  \
+        if (bs.n_max <= 8) launch_backprop<LM, 8>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);       \
+        else if (bs.n_max <= 12) launch_backprop<LM, 12>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance); \
+        else launch_backprop<LM, 16>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);                    \
         break;
-    switch (bs.l_max) {
-        FLARE_CASE(0) FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6)
-        default: break;
-    }
+        switch (bs.l_max) {
+            FLARE_CASE(0) FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6)
+            default: break;
+        }
 #undef FLARE_CASE
+    }
 }
 
 // ------------------------------------------------------------------ a7: atomics-free gather

@@ -82,7 +82,26 @@ struct GroupDesc {
     const double* sigma = nullptr;  // same or nullptr
     const int* table = nullptr;     // device [P/(l_max+1)]: pair q -> nu1 | nu2<<8; component p = q*(l_max+1) + l
     const int* lut = nullptr;       // device [Nv*Nv]: (nu1,nu2) -> pair q (symmetric), -1 if not in the group
+    unsigned mask = 0;              // neighbour species of the group (all species in dense mode)
+    int nsp = 0;                    // popcount(mask)
+    int Nc = 0;                     // nsp * n_max compact radial channels: compact index = rank(species) * n_max + n;
+                                    // the group's components are the triangular enumeration over them (x l)
+    unsigned sidx = 0;              // 4 bits per species: its rank within mask (15 = absent)
 };
+
+// What a per-(chunk, group) launch of the per-atom kernels needs (passed by value).
+struct GroupRun {
+    int g;          // group id: rows group_start[g] .. group_start[g+1], intersected with the chunk
+    int row0, nrows;  // chunk = global rows [row0, row0 + nrows)
+    int nsp, Nc;
+    unsigned sidx;
+    int P, K, ntn;
+    const int* table;
+};
+
+inline GroupRun make_group_run(const GroupDesc& gd, int g, int row0, int nrows) {
+    return GroupRun{g, row0, nrows, gd.nsp, gd.Nc, gd.sidx, gd.P, gd.K, gd.ntn, gd.table};
+}
 
 // What the per-atom kernels need to know about a group (device array indexed by group id).
 struct GroupDev {
@@ -98,17 +117,17 @@ struct GroupDev {
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
                      const int* types, int mmax, int sparse, int n_groups);
 
-// Descriptor rows [row0,row0+nrows): A -> ws.A, B^ -> bh_out (row r at (r - row0)*ld unless out_map given),
-// ||B|| -> nrm_out.  out_map (optional): row of atom k in bh_out/nrm_out is out_map[k] (used by the test hook).
+// Descriptor rows [row0,row0+nrows): compact A -> ws.A, UNNORMALISED B -> bh_out (row r at (r - row0)*ld),
+// ||B|| -> nrm_out.  One launch per group.
 void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
-                     const GroupDev* groups, int row0, int nrows, double* bh_out, int ld, double* nrm_out,
-                     const int* out_map, bool write_A);
+                     const GroupDesc* groups, int n_groups, int row0, int nrows, double* bh_out, int ld,
+                     double* nrm_out, bool write_A);
 
 void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_groups, int row0, int nrows, int ld,
                int chunk_cap, bool want_variance, int sm_count);
 
 void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
-                  const GroupDev* groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
+                  const GroupDesc* groups, int n_groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
                   bool want_variance);
 
 void run_gather(Launcher& L, const Workspace& ws, int n, int mmax, double* e_out, double* f_out, double* var_out);
