@@ -12,18 +12,17 @@
 // Epilogue (fused): energy tiles store W (needed for dE/dB) and the partial row-dot
 // sum_n W[r][n] B^[r][n]; variance tiles store only the partial row-dot.  Partials of the ntn tiles
 // of a row are summed in fixed order by the back-propagation kernel (deterministic, atomics-free).
+#include <cstdlib>
+
 #include "kernels.cuh"
 
 namespace flare {
 
-constexpr int kQfBM = 128;      // rows per CTA tile
 constexpr int kQfBK = 16;       // K slab
 constexpr int kQfLds = 20;      // padded slab row (doubles)
-constexpr int kQfStages = 4;
-constexpr int kQfThreads = 256;
 
 struct QfArgs {
-    const double* Bh;   // [chunk rows][ld]
+    const double* Bh;   // [chunk rows][ld]  (unnormalised B rows)
     double* W;          // [chunk rows][ld]
     double* part;       // [2][max_ntn][chunk_cap]
     const int* group_start;
@@ -53,19 +52,30 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-template <int NB>
-__global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
+// WARPS warps stacked along M (16 rows each): CTA tile (16 WARPS) x (8 NB).  WARPS = 4 runs two CTAs per SM
+// (3 stages each), so that one CTA's epilogue and pipeline refill overlap the other's DMMA main loop.
+template <int WARPS> struct QfCfg {
+    static constexpr int BM = 16 * WARPS;
+    static constexpr int THREADS = 32 * WARPS;
+    static constexpr int STAGES = WARPS == 8 ? 4 : 3;
+    static constexpr int MINB = WARPS == 8 ? 1 : 2;
+};
+
+template <int NB, int WARPS>
+__global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_qform(QfArgs a) {
+    using C = QfCfg<WARPS>;
     constexpr int BN = 8 * NB;
+    constexpr int BM = C::BM, THREADS = C::THREADS, STAGES = C::STAGES;
     extern __shared__ __align__(16) double smem[];
-    double* As = smem;                                     // [stages][128][20]
-    double* Bs = smem + kQfStages * kQfBM * kQfLds;        // [stages][BN][20]
+    double* As = smem;                               // [stages][BM][20]
+    double* Bs = smem + STAGES * BM * kQfLds;        // [stages][BN][20]
 
     const int gs = max(a.group_start[a.g], a.row0);
     const int ge = min(a.group_start[a.g + 1], a.row0 + a.nrows);
     const int n_rows = ge - gs;
     if (n_rows <= 0) return;
     const int lrow0 = gs - a.row0;  // first local row of this group in the chunk buffers
-    const int m_tiles = (n_rows + kQfBM - 1) / kQfBM;
+    const int m_tiles = (n_rows + BM - 1) / BM;
     const int tiles_per_m = a.ntn * a.n_mat;
     const int total = m_tiles * tiles_per_m;
 
@@ -73,15 +83,48 @@ __global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
     const int g8 = lane >> 2, t4 = lane & 3;
     const int nk = a.K / kQfBK;
 
-    for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+    // tile -> (row block, matrix, column block); loads of one K slab of a tile into a stage
+    auto load_stage = [&](int tile, int kt, int stage) {
         const int mt = tile / tiles_per_m;
         const int rem = tile - mt * tiles_per_m;
         const int mat = rem / a.ntn;
         const int nt = rem - mat * a.ntn;
         const double* M = (mat == 0 ? a.beta : a.sigma) + (size_t)nt * BN * a.K;  // rows n of the symmetric matrix
-        const int mrow0 = mt * kQfBM;  // row offset inside the group
+        const int mrow0 = mt * BM;
         const double* Ag = a.Bh + (size_t)(lrow0 + mrow0) * a.ld;
-        const int rows_here = min(kQfBM, n_rows - mrow0);
+        const int rows_here = min(BM, n_rows - mrow0);
+        const int k0 = kt * kQfBK;
+        double* as = As + stage * BM * kQfLds;
+        double* bs = Bs + stage * BN * kQfLds;
+#pragma unroll
+        for (int i = 0; i < (BM * 8) / THREADS; i++) {  // A slab: BM rows x 8 chunks of 16 B
+            const int idx = tid + i * THREADS;
+            const int r = idx >> 3, c = idx & 7;
+            const bool ok = r < rows_here;
+            const double* src = Ag + (size_t)(ok ? r : 0) * a.ld + k0 + 2 * c;
+            cp_async16(as + r * kQfLds + 2 * c, src, ok ? 16 : 0);
+        }
+        for (int idx = tid; idx < BN * 8; idx += THREADS) {  // B slab: BN rows x 8 chunks
+            const int r = idx >> 3, c = idx & 7;
+            cp_async16(bs + r * kQfLds + 2 * c, M + (size_t)r * a.K + k0 + 2 * c, 16);
+        }
+    };
+    auto prologue = [&](int tile) {
+#pragma unroll
+        for (int s = 0; s < STAGES - 1; s++) {
+            if (s < nk) load_stage(tile, s, s);
+            cp_async_commit();
+        }
+    };
+
+    int tile = blockIdx.x;
+    if (tile < total) prologue(tile);
+    while (tile < total) {
+        const int mt = tile / tiles_per_m;
+        const int rem = tile - mt * tiles_per_m;
+        const int mat = rem / a.ntn;
+        const int nt = rem - mat * a.ntn;
+        const int mrow0 = mt * BM;  // row offset inside the group
 
         double acc[2][NB][2];
 #pragma unroll
@@ -89,39 +132,13 @@ __global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
 #pragma unroll
             for (int nb = 0; nb < NB; nb++) { acc[h][nb][0] = 0.0; acc[h][nb][1] = 0.0; }
 
-        auto load_stage = [&](int kt, int stage) {
-            const int k0 = kt * kQfBK;
-            double* as = As + stage * kQfBM * kQfLds;
-            double* bs = Bs + stage * BN * kQfLds;
-            // A slab: 128 rows x 8 chunks of 16 B
-#pragma unroll
-            for (int i = 0; i < (kQfBM * 8) / kQfThreads; i++) {
-                const int idx = tid + i * kQfThreads;
-                const int r = idx >> 3, c = idx & 7;
-                const bool ok = r < rows_here;
-                const double* src = Ag + (size_t)(ok ? r : 0) * a.ld + k0 + 2 * c;
-                cp_async16(as + r * kQfLds + 2 * c, src, ok ? 16 : 0);
-            }
-            // B slab: BN rows x 8 chunks
-            for (int idx = tid; idx < BN * 8; idx += kQfThreads) {
-                const int r = idx >> 3, c = idx & 7;
-                cp_async16(bs + r * kQfLds + 2 * c, M + (size_t)r * a.K + k0 + 2 * c, 16);
-            }
-        };
-
-        __syncthreads();  // previous tile's smem reads are done
-#pragma unroll
-        for (int s = 0; s < kQfStages - 1; s++) {
-            if (s < nk) load_stage(s, s);
-            cp_async_commit();
-        }
         for (int kt = 0; kt < nk; kt++) {
-            cp_async_wait<kQfStages - 2>();
+            cp_async_wait<STAGES - 2>();
             __syncthreads();
-            if (kt + kQfStages - 1 < nk) load_stage(kt + kQfStages - 1, (kt + kQfStages - 1) % kQfStages);
+            if (kt + STAGES - 1 < nk) load_stage(tile, kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
             cp_async_commit();
-            const double* as = As + (kt % kQfStages) * kQfBM * kQfLds + (warp * 16 + g8) * kQfLds + t4;
-            const double* bs = Bs + (kt % kQfStages) * BN * kQfLds + g8 * kQfLds + t4;
+            const double* as = As + (kt % STAGES) * BM * kQfLds + (warp * 16 + g8) * kQfLds + t4;
+            const double* bs = Bs + (kt % STAGES) * BN * kQfLds + g8 * kQfLds + t4;
 #pragma unroll
             for (int ks = 0; ks < kQfBK / 4; ks++) {
                 const double a0 = as[4 * ks];
@@ -134,9 +151,13 @@ __global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
                 }
             }
         }
-        cp_async_wait<0>();
+        // all warps are done with the stages: refill the pipeline for the next tile, so that its first
+        // slabs arrive while this tile's epilogue runs
+        __syncthreads();
+        const int next = tile + gridDim.x;
+        if (next < total) prologue(next);
 
-        // ---- fused epilogue: W store (energy tiles) + partial row-dot with B^ of the same columns
+        // ---- fused epilogue: W store (energy tiles) + partial row-dot with B of the same columns
         const int n0 = nt * BN;
         double* part = a.part + ((size_t)mat * a.max_ntn + nt) * a.chunk_cap;
 #pragma unroll
@@ -146,16 +167,33 @@ __global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
             const size_t lrow = (size_t)(lrow0 + r);
             double dot = 0.0;
             if (rok) {
-                const double* brow = a.Bh + lrow * a.ld;
-                double* wrow = a.W + lrow * a.ld;
+                const double* __restrict__ brow = a.Bh + lrow * a.ld;
+                double* __restrict__ wrow = a.W + lrow * a.ld;
+                // the B loads of a batch are issued together (one L2 round trip per batch, not per column block)
+                constexpr int CH = 6;
 #pragma unroll
-                for (int nb = 0; nb < NB; nb++) {
-                    const int n = n0 + nb * 8 + 2 * t4;
-                    if (n < a.K) {  // K is even, so n+1 < K too
-                        const double2 bv = *reinterpret_cast<const double2*>(brow + n);
-                        dot = fma(acc[h][nb][0], bv.x, dot);
-                        dot = fma(acc[h][nb][1], bv.y, dot);
-                        if (mat == 0) *reinterpret_cast<double2*>(wrow + n) = make_double2(acc[h][nb][0], acc[h][nb][1]);
+                for (int nb0 = 0; nb0 < NB; nb0 += CH) {
+                    double2 bv[CH];
+#pragma unroll
+                    for (int c = 0; c < CH; c++) {
+                        const int n = n0 + (nb0 + c) * 8 + 2 * t4;
+                        bv[c] = (nb0 + c < NB && n < a.K) ? __ldg(reinterpret_cast<const double2*>(brow + n))
+                                                          : make_double2(0.0, 0.0);
+                    }
+#pragma unroll
+                    for (int c = 0; c < CH; c++) {
+                        if (nb0 + c < NB) {
+                            dot = fma(acc[h][nb0 + c][0], bv[c].x, dot);
+                            dot = fma(acc[h][nb0 + c][1], bv[c].y, dot);
+                        }
+                    }
+                }
+                if (mat == 0) {
+#pragma unroll
+                    for (int nb = 0; nb < NB; nb++) {
+                        const int n = n0 + nb * 8 + 2 * t4;
+                        if (n < a.K)  // K is even, so n+1 < K too
+                            *reinterpret_cast<double2*>(wrow + n) = make_double2(acc[h][nb][0], acc[h][nb][1]);
                     }
                 }
             }
@@ -163,19 +201,35 @@ __global__ void __launch_bounds__(kQfThreads, 1) k_qform(QfArgs a) {
             dot += __shfl_xor_sync(kFull, dot, 2);
             if (rok && t4 == 0) part[lrow] = dot;
         }
+        tile = next;
     }
+    cp_async_wait<0>();
 }
 
-template <int NB>
-static void launch_qform(Launcher& L, const QfArgs& a, int grid) {
+static int qf_variant() {  // development knob: FLARE_QF_WARPS=8 selects the 128-row, one-CTA-per-SM tiling
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("FLARE_QF_WARPS");
+        v = (e && atoi(e) == 8) ? 8 : 4;
+    }
+    return v;
+}
+
+template <int NB, int WARPS>
+static void launch_qform(Launcher& L, const QfArgs& a, int sm_count, long long max_m_rows) {
+    using C = QfCfg<WARPS>;
     constexpr int BN = 8 * NB;
-    const size_t smem = sizeof(double) * kQfStages * (kQfBM + BN) * kQfLds;
+    const size_t smem = sizeof(double) * C::STAGES * (C::BM + BN) * kQfLds;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_qform<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_qform<NB, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
-    L.launch(k_qform<NB>, dim3(grid), dim3(kQfThreads), smem, a);
+    // persistent grid: MINB CTAs per SM, but never more CTAs than the chunk could give tiles
+    const long long max_tiles = ((max_m_rows + C::BM - 1) / C::BM) * a.ntn * a.n_mat;
+    const long long cap = (long long)sm_count * C::MINB;
+    const int grid = (int)(max_tiles < cap ? max_tiles : cap);
+    L.launch(k_qform<NB, WARPS>, dim3(grid), dim3(C::THREADS), smem, a);
 }
 
 void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_groups, int row0, int nrows, int ld,
@@ -183,6 +237,7 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
     if (nrows <= 0) return;
     int max_ntn = 0;
     for (int g = 0; g < n_groups; g++) max_ntn = groups[g].ntn > max_ntn ? groups[g].ntn : max_ntn;
+    const int variant = qf_variant();
     for (int g = 0; g < n_groups; g++) {
         const GroupDesc& gd = groups[g];
         if (gd.K == 0 || gd.beta == nullptr) continue;
@@ -192,11 +247,12 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
         a.g = g; a.row0 = row0; a.nrows = nrows; a.ld = ld; a.K = gd.K; a.ntn = gd.ntn;
         a.n_mat = (want_variance && gd.sigma) ? 2 : 1;
         a.chunk_cap = chunk_cap; a.max_ntn = max_ntn;
-        // persistent grid: one CTA per SM, but never more CTAs than the chunk could give tiles
-        long long max_tiles = (long long)((nrows + kQfBM - 1) / kQfBM) * gd.ntn * a.n_mat;
-        int grid = (int)(max_tiles < sm_count ? max_tiles : sm_count);
         switch (gd.nb) {
-#define FLARE_CASE(NBV) case NBV: launch_qform<NBV>(L, a, grid); break;
+#define FLARE_CASE(NBV)                                                   \
+    case NBV:                                                             \
+        if (variant == 8) launch_qform<NBV, 8>(L, a, sm_count, nrows);    \
+        else launch_qform<NBV, 4>(L, a, sm_count, nrows);                 \
+        break;
             FLARE_CASE(2) FLARE_CASE(4) FLARE_CASE(6) FLARE_CASE(8) FLARE_CASE(9) FLARE_CASE(10) FLARE_CASE(11)
             FLARE_CASE(12) FLARE_CASE(13) FLARE_CASE(14) FLARE_CASE(15) FLARE_CASE(16) FLARE_CASE(17) FLARE_CASE(18)
 #undef FLARE_CASE
