@@ -283,9 +283,10 @@ def run_ours(args):
     roofline = {
         "bound": "tensor", "kernel": "k_qform (FP64 DMMA grouped GEMM, beta + Sigma forms)",
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
-        # dram__bytes_read+write of k_qform per atom row, from the ncu --set full capture in
-        # profiles/r01_qform_full.md (1.771 GB for the 205 184-row launch), scaled to one step's rows
-        "traffic": 8630.0 * n if (P == 544 and not sparse) else None,
+        # dram__bytes_read+write of k_qform per row, from the ncu --set full capture in profiles/r01c_qform_full.md
+        # (2 251 B per K=144 row, 5 556 B per K=544 row, variance on), scaled to one step's rows
+        "traffic": (float(sum(r * {144: 2251.0, 544: 5556.0}[p] for r, p in groups))
+                    if want_var and all(p in (144, 544) for _, p in groups) else None),
         "algorithmic_bytes": qf_bytes_per_step,
         "groups_rows_x_components": groups,
         "peak_source": "FP64 DMMA issue peak measured live by flare_measure_fp64_dmma_peak "

@@ -606,9 +606,9 @@ int oracle_descriptor(int64_t N, const double *pos, const int32_t *types, const 
  *   F_i += g_ij,  F_j -= g_ij   with g_ij = dE_i/dr_ij, r_ij = x_j - x_i
  * e_out/f_out/v_out may each be NULL.  nbr_method: 0 brute force, 1 cell grid.
  */
-int oracle_compute(int64_t N, const double *pos, const int32_t *types, const double box[9], const int pbc[3],
-                   int S, int n_max, int l_max, const double *r_cut, const double *beta, const double *sigma,
-                   int nbr_method, double *e_out, double *f_out, double *v_out)
+static int compute_impl(int64_t N, const double *pos, const int32_t *types, const double box[9], const int pbc[3],
+                        int S, int n_max, int l_max, const double *r_cut, const double *beta, const double *sigma,
+                        int nbr_method, double *e_out, double *f_out, double *v_out, double *vir_out)
 {
     model_t md = {S, n_max, l_max, r_cut, beta, sigma};
     int rc = check_system(box, pbc, S, r_cut);
@@ -622,7 +622,7 @@ int oracle_compute(int64_t N, const double *pos, const int32_t *types, const dou
     rc = build_nlist(N, xw, types, box, pbc, S, r_cut, nbr_method, &nl);
     if (rc) { free(xw); return rc; }
     int64_t npair = nl.off[N];
-    double *gpair = f_out ? (double *)malloc(sizeof(double) * 3 * (size_t)(npair > 0 ? npair : 1)) : NULL;
+    double *gpair = (f_out || vir_out) ? (double *)malloc(sizeof(double) * 3 * (size_t)(npair > 0 ? npair : 1)) : NULL;
     int64_t mmax = 0;
     for (int64_t i = 0; i < N; i++) if (nl.off[i + 1] - nl.off[i] > mmax) mmax = nl.off[i + 1] - nl.off[i];
 
@@ -658,9 +658,80 @@ int oracle_compute(int64_t N, const double *pos, const int32_t *types, const dou
                 }
             }
     }
+    if (vir_out) {
+        /* Xi_ab = dE/d eps_ab under x -> (1 + eps) x: every r_ij -> (1 + eps) r_ij, so
+           Xi_ab = sum_i sum_{j in N(i)} (dE_i/dr_ij)_a (r_ij)_b      (stress) */
+        for (int a = 0; a < 9; a++) vir_out[a] = 0.0;
+        for (int64_t i = 0; i < N; i++)
+            for (int64_t q = nl.off[i]; q < nl.off[i + 1]; q++) {
+                double d[3];
+                min_image(xw + 3 * i, xw + 3 * nl.idx[q], box, pbc, d);
+                for (int a = 0; a < 3; a++)
+                    for (int b = 0; b < 3; b++) vir_out[3 * a + b] += gpair[3 * q + a] * d[b];
+            }
+    }
     free(gpair);
     nlist_free(&nl);
     free(xw);
+    return ORACLE_OK;
+}
+
+int oracle_compute(int64_t N, const double *pos, const int32_t *types, const double box[9], const int pbc[3],
+                   int S, int n_max, int l_max, const double *r_cut, const double *beta, const double *sigma,
+                   int nbr_method, double *e_out, double *f_out, double *v_out)
+{
+    return compute_impl(N, pos, types, box, pbc, S, n_max, l_max, r_cut, beta, sigma, nbr_method, e_out, f_out, v_out,
+                        NULL);
+}
+
+/* Exported: oracle_compute plus the virial Xi[3a+b] = dE/d eps_ab (eV); potential stress = Xi / volume. */
+int oracle_compute_virial(int64_t N, const double *pos, const int32_t *types, const double box[9], const int pbc[3],
+                          int S, int n_max, int l_max, const double *r_cut, const double *beta, const double *sigma,
+                          int nbr_method, double *e_out, double *f_out, double *v_out, double *vir_out)
+{
+    return compute_impl(N, pos, types, box, pbc, S, n_max, l_max, r_cut, beta, sigma, nbr_method, e_out, f_out, v_out,
+                        vir_out);
+}
+
+/*
+ * Exported: the on-the-fly analysis of the paper's production run ("coordination numbers of H atoms ...
+ * another H within 1 A"; "monitoring the maximum uncertainty"):
+ *   max_unc = max_i sqrt(max(V_i, 0)); n_above = #{i : sqrt(max(V_i,0)) > threshold}
+ *   coord[i] = #{j != i : s_j = species_b, |r_ij|^2 < r_coord^2 (minimum image)} if s_i = species_a, else 0
+ * by brute force over all pairs.
+ */
+int oracle_analyze(int64_t N, const double *pos, const int32_t *types, const double box[9], const int pbc[3],
+                   const double *var, double threshold, int species_a, int species_b, double r_coord,
+                   double *max_unc, int64_t *n_above, int32_t *coord)
+{
+    if (!box_is_orthorhombic(box)) return ORACLE_ERR_BOX;
+    double mx = 0.0;
+    int64_t na = 0;
+    if (var)
+        for (int64_t i = 0; i < N; i++) {
+            double u = sqrt(var[i] > 0.0 ? var[i] : 0.0);
+            if (u > mx) mx = u;
+            if (u > threshold) na++;
+        }
+    if (max_unc) *max_unc = mx;
+    if (n_above) *n_above = na;
+    if (coord) {
+        double *xw = (double *)malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
+        if (!xw) return ORACLE_ERR_NOMEM;
+        oracle_wrap(N, pos, box, pbc, xw);
+        for (int64_t i = 0; i < N; i++) {
+            int32_t c = 0;
+            if (types[i] == species_a)
+                for (int64_t j = 0; j < N; j++) {
+                    double d[3];
+                    if (j == i || types[j] != species_b) continue;
+                    min_image(xw + 3 * i, xw + 3 * j, box, pbc, d);
+                    if (dist2(d) < r_coord * r_coord) c++;
+                }
+            coord[i] = c;
+        }
+        free(xw);
+    }
     return ORACLE_OK;
 }
 
@@ -772,5 +843,76 @@ int oracle_step(int64_t N, double *pos, double *vel, const int32_t *types, const
     if (f_out) memcpy(f_out, F, sizeof(double) * 3 * (size_t)N);
     if (v_out) memcpy(v_out, V, sizeof(double) * (size_t)N);
     free(E); free(F); free(V);
+    return rc;
+}
+
+/* ------------------------------------------------------------------ Nose-Hoover NVT (R19) */
+
+#define KB_EV 8.617333262e-5 /* eV/K (R13) */
+
+/* half step of the single Nose-Hoover thermostat (Martyna-Tuckerman-Klein splitting), h = dt/2:
+ *   xi += (h/2)(K2 - g kT)/Q ;  v *= exp(-xi h) ;  eta += xi h ;  xi += (h/2)(K2' - g kT)/Q
+ * with K2 = sum m v^2 / kappa (twice the kinetic energy, eV), Q = g kT tau^2, g = 3N - 3. */
+static void nh_half(int64_t N, double *vel, const int32_t *types, const double *mass, double h, double gkT, double Q,
+                    double *xi, double *eta)
+{
+    double K2 = 0.0;
+    for (int64_t i = 0; i < N; i++)
+        for (int d = 0; d < 3; d++) K2 += mass[types[i]] * vel[3 * i + d] * vel[3 * i + d] / KAPPA;
+    *xi += 0.5 * h * (K2 - gkT) / Q;
+    double s = exp(-(*xi) * h);
+    for (int64_t a = 0; a < 3 * N; a++) vel[a] *= s;
+    K2 *= s * s;
+    *eta += (*xi) * h;
+    *xi += 0.5 * h * (K2 - gkT) / Q;
+}
+
+/*
+ * n_steps of: thermostat half step ; velocity Verlet (as oracle_step) ; thermostat half step.
+ * xi_eta[2] = {xi (1/fs), eta} is read and updated.  cons_trace [n_steps+1]: the conserved quantity
+ * KE + PE + Q xi^2 / 2 + g kT eta after 0..n_steps steps; temp_trace: 2 KE / (g k_B).
+ */
+int oracle_step_nvt(int64_t N, double *pos, double *vel, const int32_t *types, const double *mass,
+                    const double box[9], const int pbc[3], int S, int n_max, int l_max, const double *r_cut,
+                    const double *beta, const double *sigma, int nbr_method, double dt, int n_steps, double T_target,
+                    double tau, double *xi_eta, double *e_out, double *f_out, double *cons_trace, double *temp_trace)
+{
+    if (N < 2 || !(T_target > 0.0) || !(tau > 0.0)) return ORACLE_ERR_ARG;
+    double *E = (double *)malloc(sizeof(double) * (size_t)N);
+    double *F = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    if (!E || !F) return ORACLE_ERR_NOMEM;
+    const double g = 3.0 * (double)N - 3.0;
+    const double gkT = g * KB_EV * T_target;
+    const double Q = gkT * tau * tau;
+    double xi = xi_eta[0], eta = xi_eta[1];
+    oracle_wrap(N, pos, box, pbc, pos);
+    int rc = oracle_compute(N, pos, types, box, pbc, S, n_max, l_max, r_cut, beta, sigma, nbr_method, E, F, NULL);
+    for (int step = 0; rc == ORACLE_OK && step <= n_steps; step++) {
+        double pe = 0.0, ke = 0.0;
+        for (int64_t i = 0; i < N; i++) {
+            pe += E[i];
+            for (int d = 0; d < 3; d++) ke += 0.5 * mass[types[i]] * vel[3 * i + d] * vel[3 * i + d] / KAPPA;
+        }
+        if (cons_trace) cons_trace[step] = ke + pe + 0.5 * Q * xi * xi + gkT * eta;
+        if (temp_trace) temp_trace[step] = 2.0 * ke / (g * KB_EV);
+        if (step == n_steps) break;
+        nh_half(N, vel, types, mass, 0.5 * dt, gkT, Q, &xi, &eta);
+        for (int64_t i = 0; i < N; i++)
+            for (int d = 0; d < 3; d++) {
+                vel[3 * i + d] += 0.5 * dt * KAPPA * F[3 * i + d] / mass[types[i]];
+                pos[3 * i + d] += dt * vel[3 * i + d];
+            }
+        oracle_wrap(N, pos, box, pbc, pos);
+        rc = oracle_compute(N, pos, types, box, pbc, S, n_max, l_max, r_cut, beta, sigma, nbr_method, E, F, NULL);
+        if (rc) break;
+        for (int64_t i = 0; i < N; i++)
+            for (int d = 0; d < 3; d++) vel[3 * i + d] += 0.5 * dt * KAPPA * F[3 * i + d] / mass[types[i]];
+        nh_half(N, vel, types, mass, 0.5 * dt, gkT, Q, &xi, &eta);
+    }
+    xi_eta[0] = xi;
+    xi_eta[1] = eta;
+    if (e_out) memcpy(e_out, E, sizeof(double) * (size_t)N);
+    if (f_out) memcpy(f_out, F, sizeof(double) * 3 * (size_t)N);
+    free(E); free(F);
     return rc;
 }

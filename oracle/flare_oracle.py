@@ -240,3 +240,53 @@ def step(pos, vel, types, mass, box, pbc, n_max, l_max, r_cut, beta, sigma, dt, 
                            C.c_int(nbr_method), C.c_double(dt), C.c_int(n_steps), _p(E), _p(F), _p(V), _p(pe), _p(ke))
     _check(rc, "oracle_step")
     return dict(pos=pos, vel=vel, E=E, F=F, V=V, pe=pe, ke=ke)
+
+
+def compute_virial(pos, types, box, pbc, n_max, l_max, r_cut, beta, sigma=None, nbr_method: int = 1):
+    """E [N], F [N,3], V [N] and the virial Xi [3,3] = dE/d eps (eV); potential stress = Xi / volume."""
+    pos = _f64(pos).reshape(-1, 3)
+    types = _i32(types)
+    N = pos.shape[0]
+    S, r_cut, beta, sigma = _model_args(n_max, l_max, r_cut, beta, sigma)
+    E, F, V, W = np.zeros(N), np.zeros((N, 3)), np.zeros(N), np.zeros(9)
+    rc = lib().oracle_compute_virial(C.c_int64(N), _p(pos), _p(types), _p(_box9(box)), _p(_pbc3(pbc)), C.c_int(S),
+                                     C.c_int(n_max), C.c_int(l_max), _p(r_cut), _p(beta), _p(sigma),
+                                     C.c_int(nbr_method), _p(E), _p(F), _p(V), _p(W))
+    _check(rc, "oracle_compute_virial")
+    return E, F, V, W.reshape(3, 3)
+
+
+def analyze(pos, types, box, pbc, var, threshold, species_a, species_b, r_coord):
+    """(max sqrt(V), #atoms with sqrt(V) > threshold, coordination numbers [N]) by brute force."""
+    pos = _f64(pos).reshape(-1, 3)
+    types = _i32(types)
+    N = pos.shape[0]
+    var = None if var is None else _f64(var)
+    mx = C.c_double(0.0)
+    na = C.c_int64(0)
+    coord = np.zeros(N, dtype=np.int32)
+    rc = lib().oracle_analyze(C.c_int64(N), _p(pos), _p(types), _p(_box9(box)), _p(_pbc3(pbc)), _p(var),
+                              C.c_double(threshold), C.c_int(species_a), C.c_int(species_b), C.c_double(r_coord),
+                              C.byref(mx), C.byref(na), _p(coord))
+    _check(rc, "oracle_analyze")
+    return mx.value, na.value, coord
+
+
+def step_nvt(pos, vel, types, mass, box, pbc, n_max, l_max, r_cut, beta, dt, n_steps, T_target, tau, xi_eta=(0.0, 0.0),
+             nbr_method: int = 1):
+    """Nose-Hoover NVT.  Returns dict(pos, vel, E, F, xi, eta, cons[n_steps+1], temp[n_steps+1])."""
+    pos = _f64(pos).reshape(-1, 3).copy()
+    vel = _f64(vel).reshape(-1, 3).copy()
+    types = _i32(types)
+    mass = _f64(mass)
+    N = pos.shape[0]
+    S, r_cut, beta, _ = _model_args(n_max, l_max, r_cut, beta, None)
+    E, F = np.zeros(N), np.zeros((N, 3))
+    xe = _f64(np.array(xi_eta, dtype=np.float64))
+    cons, temp = np.zeros(n_steps + 1), np.zeros(n_steps + 1)
+    rc = lib().oracle_step_nvt(C.c_int64(N), _p(pos), _p(vel), _p(types), _p(mass), _p(_box9(box)), _p(_pbc3(pbc)),
+                               C.c_int(S), C.c_int(n_max), C.c_int(l_max), _p(r_cut), _p(beta), None,
+                               C.c_int(nbr_method), C.c_double(dt), C.c_int(n_steps), C.c_double(T_target),
+                               C.c_double(tau), _p(xe), _p(E), _p(F), _p(cons), _p(temp))
+    _check(rc, "oracle_step_nvt")
+    return dict(pos=pos, vel=vel, E=E, F=F, xi=float(xe[0]), eta=float(xe[1]), cons=cons, temp=temp)

@@ -24,10 +24,20 @@ struct BpSmem {
     static constexpr int L2 = (LMAX + 1) * (LMAX + 1);
     static constexpr int AS = bp_pad4mod16(L2);    // row stride of the staged A (conflict-free operand loads)
     static constexpr int GB = L2 * NMAXP + 2;      // G^T block of one (atom, species): [L2][NMAXP] + bank shift
+    // G^T of ta atoms + double-buffered [A | W | B] rows of one atom (filled by cp.async one atom ahead)
     __host__ __device__ static int warp_doubles(int ta, int nsp, int Nc8, int K) {
-        return (ta * nsp * GB + Nc8 * AS + K + 1) & ~1;  // even: every warp's region stays 16-byte aligned
+        return (ta * nsp * GB + 2 * (Nc8 * AS + 2 * K) + 1) & ~1;  // even: every warp's region stays 16-byte aligned
     }
 };
+
+__device__ __forceinline__ void bp_cp_async16(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src));
+}
+__device__ __forceinline__ void bp_cp_async8(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gmem_src));
+}
 
 __device__ __forceinline__ void dmma884_f(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -88,9 +98,9 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     const int n_max = bs.n_max;
     const int Nc = gr.Nc, Nc8 = (Nc + 7) & ~7, nmb = Nc8 >> 3;
     double* Gt = smem + (size_t)warp * SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);  // [ta][nsp][GB]
-    double* As = Gt + ta * gr.nsp * GB;                                           // [Nc8][AS]
-    double* cs = As + Nc8 * AS;                                                   // [K]
-    for (int c = lane; c < ta * gr.nsp * GB + Nc8 * AS; c += 32) Gt[c] = 0.0;  // G^T (n >= n_max stays 0) and A
+    double* rows = Gt + ta * gr.nsp * GB;  // [2][ A [Nc8][AS] | W [K] | B [K] ]
+    const int row_doubles = Nc8 * AS + 2 * gr.K;
+    for (int c = lane; c < ta * gr.nsp * GB + 2 * row_doubles; c += 32) Gt[c] = 0.0;  // G^T (n >= n_max stays 0), A padding
 
     int my_k = 0, my_cnt = 0;
     if (lane < na) {
@@ -107,37 +117,73 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     const int T = __shfl_sync(kFull, my_end, kBpMaxTA - 1);
     __syncwarp();
 
+    // Phase-2 loads (neighbour index, then the two atoms) are issued one pass ahead of their use; the first
+    // pass's already here, so that they fly during phase 1.
+    auto locate = [&](int p, int& ai, int& k, int& s) {
+        ai = 0;
+#pragma unroll
+        for (int i = 0; i < kBpMaxTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
+        k = __shfl_sync(kFull, my_k, ai);
+        s = p - __shfl_sync(kFull, my_start, ai);
+    };
+    int ai_n, k_n, s_n, j_n = 0;
+    locate(lane, ai_n, k_n, s_n);
+    if (lane < T) j_n = nbr_idx[(size_t)k_n * mmax + s_n];
+    AtomS me_n = load_atom(atoms + k_n), o_n = load_atom(atoms + j_n);
+
     // ---------------- phase 1: per atom E, V, c, G
-    for (int a = 0; a < na; a++) {
-        const int k = __shfl_sync(kFull, my_k, a);
-        const int lrow = lrow0 + a;
-        // E, V from the tile partials (fixed order => deterministic); the rows hold the unnormalised B,
-        // so E = B^T beta B / ||B||^2 and c = dE/dB = (2/||B||^2)(W - E B) with W = beta B   (R10, R11)
+    // E, V from the tile partials (fixed order => deterministic), lane a for atom a so that the loads of all
+    // atoms are in flight together; the rows hold the unnormalised B, so E = B^T beta B / ||B||^2 and
+    // c = dE/dB = (2/||B||^2)(W - E B) with W = beta B   (R10, R11)
+    double my_E = 0.0, my_inv2 = 0.0;
+    if (lane < na) {
+        const int lrow = lrow0 + lane;
         double E = 0.0, V = 0.0;
         for (int t = 0; t < gr.ntn; t++) E += part[(size_t)t * chunk_cap + lrow];
         if (want_variance)
             for (int t = 0; t < gr.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + lrow];
         const double nrm = (gr.P > 0) ? nrm_in[lrow] : 0.0;
-        const double inv2 = (nrm > 0.0) ? 1.0 / (nrm * nrm) : 0.0;  // no neighbours: E = V = 0 (R8)
-        E *= inv2;
-        V *= inv2;
-        if (lane == 0) { e_s[k] = E; v_s[k] = V; }
-        if (gr.P == 0) continue;
-
+        my_inv2 = (nrm > 0.0) ? 1.0 / (nrm * nrm) : 0.0;  // no neighbours: E = V = 0 (R8)
+        my_E = E * my_inv2;
+        e_s[my_k] = my_E;
+        v_s[my_k] = V * my_inv2;
+    }
+    // A (compact, into its padded layout), W = beta B and B of one atom -> shared memory, asynchronously
+    auto issue_rows = [&](int a, int buf) {
+        const int lrow = lrow0 + a;
+        double* As = rows + buf * row_doubles;
         const double* arow = A_in + (size_t)lrow * bs.NvL2;
-        for (int c = lane; c < Nc * L2; c += 32) {
-            const int nu = c / L2;
-            As[nu * AS + (c - nu * L2)] = arow[c];
+        if constexpr (L2 % 2 == 0) {
+            for (int c = 2 * lane; c < Nc * L2; c += 64) {
+                const int nu = c / L2;
+                bp_cp_async16(As + nu * AS + (c - nu * L2), arow + c);
+            }
+        } else {
+            for (int c = lane; c < Nc * L2; c += 32) {
+                const int nu = c / L2;
+                bp_cp_async8(As + nu * AS + (c - nu * L2), arow + c);
+            }
         }
+        double* Ws = As + Nc8 * AS;
         const double* wrow = W + (size_t)lrow * ld;
         const double* brow = Braw + (size_t)lrow * ld;
-        const double two_inv2 = 2.0 * inv2;
-        for (int p = lane; p < gr.P; p += 32) {
-            const int t = __ldg(gr.table + p / L);
-            const double dbl = ((t & 255) == (t >> 8)) ? 2.0 : 1.0;  // the (1 + delta) factor of the diagonal pairs
-            cs[p] = dbl * two_inv2 * (wrow[p] - E * brow[p]);
+        for (int c = 2 * lane; c < gr.K; c += 64) {
+            bp_cp_async16(Ws + c, wrow + c);
+            bp_cp_async16(Ws + gr.K + c, brow + c);
         }
+    };
+    if (gr.P > 0) issue_rows(0, 0);
+    asm volatile("cp.async.commit_group;\n" ::);
+    for (int a = 0; a < na && gr.P > 0; a++) {
+        if (a + 1 < na) issue_rows(a + 1, (a + 1) & 1);
+        asm volatile("cp.async.commit_group;\n" ::);
+        asm volatile("cp.async.wait_group 1;\n" ::);
         __syncwarp();
+        const double E = __shfl_sync(kFull, my_E, a);
+        const double two_inv2 = 2.0 * __shfl_sync(kFull, my_inv2, a);
+        const double* As = rows + (a & 1) * row_doubles;
+        const double* Ws = As + Nc8 * AS;
+        const double* Bs = Ws + gr.K;
 
         // G[cnu1, (l,m)] = sum_cnu2 C_l[cnu1,cnu2] A[cnu2,(l,m)], C_l[cnu1,cnu2] = c[q(cnu1,cnu2) L + l]: per l a small
         // symmetric-matrix product on the tensor pipe.  A-operand (row cnu1 = 8mb+g8, col cnu2 = k0+t4),
@@ -154,11 +200,12 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
                 const int nu2 = k0 + t4;
                 const bool in = nu1 < Nc && nu2 < Nc;
                 const int lo = min(nu1, nu2), hi = max(nu1, nu2);
-                const double* cq = cs + (in ? (lo * Nc - (lo * (lo - 1)) / 2 + (hi - lo)) * L : 0);
+                const int cq = in ? (lo * Nc - (lo * (lo - 1)) / 2 + (hi - lo)) * L : 0;
+                const double fac = (nu1 == nu2) ? 2.0 * two_inv2 : two_inv2;  // (1 + delta) of the diagonal pairs
                 const double* a2 = As + nu2 * AS + g8;
 #pragma unroll
                 for (int l = 0; l < L; l++) {
-                    const double av = in ? cq[l] : 0.0;
+                    const double av = in ? fac * (Ws[cq + l] - E * Bs[cq + l]) : 0.0;  // c = dE/dB
 #pragma unroll
                     for (int nb = 0; nb < NBL; nb++) {
                         if (nb * 8 < 2 * l + 1) {
@@ -187,15 +234,15 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     // ---------------- phase 2: per-pair forces f_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj), one pair per lane
     for (int p0 = 0; p0 < T; p0 += 32) {
         const int p = p0 + lane;
-        int ai = 0;
-#pragma unroll
-        for (int i = 0; i < kBpMaxTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
-        const int k = __shfl_sync(kFull, my_k, ai);
-        const int s = p - __shfl_sync(kFull, my_start, ai);
+        const int ai = ai_n, k = k_n, s = s_n;
+        const AtomS me = me_n, o = o_n;
+        if (p0 + 32 < T) {  // uniform
+            locate(p + 32, ai_n, k_n, s_n);
+            j_n = (p + 32 < T) ? nbr_idx[(size_t)k_n * mmax + s_n] : 0;
+            me_n = load_atom(atoms + k_n);
+            o_n = load_atom(atoms + j_n);
+        }
         if (p < T) {
-            const int j = nbr_idx[(size_t)k * mmax + s];
-            const AtomS me = load_atom(atoms + k);
-            const AtomS o = load_atom(atoms + j);
             double dx, dy, dz;
             displacement(g, me, o, dx, dy, dz);
             const double r2 = dx * dx + dy * dy + dz * dz;
@@ -209,15 +256,18 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
             double srad = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
             real_ylm<LMAX, true>(yn, ux, uy, uz, [&](int lm, double Y, double gx, double gy, double gz) {
                 const double2* gp = reinterpret_cast<const double2*>(Gj + lm * NMAXP);
-                double hr = 0.0, hg = 0.0;  // sum_n G[n,lm] dg_n  and  sum_n G[n,lm] g_n
+                // sum_n G[n,lm] dg_n  and  sum_n G[n,lm] g_n, as four independent chains
+                double hr = 0.0, hg = 0.0, hr1 = 0.0, hg1 = 0.0;
 #pragma unroll
                 for (int n2 = 0; n2 < NMAXP / 2; n2++) {
                     const double2 Gv = gp[n2];
                     hr = fma(Gv.x, dgr[2 * n2], hr);
-                    hr = fma(Gv.y, dgr[2 * n2 + 1], hr);
+                    hr1 = fma(Gv.y, dgr[2 * n2 + 1], hr1);
                     hg = fma(Gv.x, gr_[2 * n2], hg);
-                    hg = fma(Gv.y, gr_[2 * n2 + 1], hg);
+                    hg1 = fma(Gv.y, gr_[2 * n2 + 1], hg1);
                 }
+                hr += hr1;
+                hg += hg1;
                 srad = fma(hr, Y, srad);
                 vx = fma(hg, gx, vx);
                 vy = fma(hg, gy, vy);
@@ -241,7 +291,7 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
     // atoms per warp: as many as keep a warp's shared memory near 14 KB (4 CTAs per SM), at least 1, at most 8
     int ta = kBpMaxTA;
     if (gr.nsp > 0) {
-        const int budget = 1792 - (Nc8 * SM::AS + gr.K);
+        const int budget = 1792 - 2 * (Nc8 * SM::AS + 2 * gr.K);
         ta = budget / (gr.nsp * SM::GB);
         ta = ta < 1 ? 1 : (ta > kBpMaxTA ? kBpMaxTA : ta);
     }
