@@ -156,6 +156,39 @@ int flare_set_forces_host(flare_ctx* ctx, const double* f);
  */
 int flare_step(flare_ctx* ctx, double dt_fs, int n_steps, int want_variance);
 
+/*
+ * The same with a Nose-Hoover thermostat (the paper's production integrator; R19): every
+ * step is bracketed by two thermostat half steps of length h = dt/2,
+ *     xi += (h/2)(K2 - g kT)/Q ;  v *= exp(-xi h) ;  eta += xi h ;  xi += (h/2)(K2' - g kT)/Q,
+ * K2 = sum m v^2 / KAPPA (eV), g = 3N - 3, Q = g k_B T tau^2, k_B = 8.617333262e-5 eV/K.  The thermostat state
+ * (xi in 1/fs, eta) lives on the device (zeroed by flare_bind) and is read / set by the two calls below
+ * (both synchronise).  Conserved: KE + sum E_i + Q xi^2/2 + g k_B T eta.  Asynchronous like flare_step.
+ */
+int flare_step_nvt(flare_ctx* ctx, double dt_fs, int n_steps, int want_variance, double T_kelvin, double tau_fs);
+int flare_get_thermostat(flare_ctx* ctx, double* xi, double* eta);
+int flare_set_thermostat(flare_ctx* ctx, double xi, double eta);
+
+/*
+ * Virial of the last evaluation (the model predicts "energy, forces and stress"):
+ *     virial[3a+b] = dE/d eps_ab = sum_i sum_{j in N(i)} (dE_i/dr_ij)_a (r_ij)_b      (eV, symmetric),
+ * reduced from the per-pair forces the evaluation stored; potential stress = virial / volume.  HOST output.
+ * Synchronises.  Deterministic (fixed summation order).
+ */
+int flare_get_virial(flare_ctx* ctx, double virial[9]);
+
+/*
+ * On-the-fly analysis of the last evaluation, as in the paper's production run:
+ *   max_unc     max_i sqrt(max(V_i, 0)) (the "maximum uncertainty"); n_above = #{i : sqrt(V_i) > unc_threshold}
+ *               (both need an evaluation with variances, else FLARE_ERR_INVALID_ARG)
+ *   coord       [N] device int32 or NULL: for atoms of species_a the number of neighbours of species_b with
+ *               |r_ij| < r_coord (the paper: H atoms with another H within 1 A), 0 for other atoms;
+ *               0 < r_coord <= r_cut[a][b] because the neighbour list is what is searched
+ *   coord_hist  [16] host or NULL: histogram of those numbers over the species_a atoms (last bin: >= 15)
+ * max_unc, n_above, coord_hist are HOST pointers; any output may be NULL.  Synchronises.
+ */
+int flare_analyze(flare_ctx* ctx, double unc_threshold, int species_a, int species_b, double r_coord,
+                  double* max_unc, int64_t* n_above, int32_t* coord, int64_t* coord_hist);
+
 /* Copy the state out; any pointer may be NULL.  Device-pointer version is asynchronous. */
 int flare_get_state(flare_ctx* ctx, double* pos, double* vel, double* e, double* f, double* var);
 int flare_get_state_host(flare_ctx* ctx, double* pos, double* vel, double* e, double* f, double* var);

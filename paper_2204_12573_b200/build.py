@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libflare_b200.so")
-SOURCES = ["flare_api.cu", "neighbor.cu", "descriptor.cu", "qform.cu", "force.cu", "integrate.cu"]
+SOURCES = ["flare_api.cu", "neighbor.cu", "descriptor.cu", "qform.cu", "force.cu", "integrate.cu", "analysis.cu"]
 HEADERS = ["common.cuh", "basis.cuh", "kernels.cuh", os.path.join("..", "..", "include", "flare_b200.h")]
 NVCC = os.environ.get("NVCC", "nvcc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -48,6 +48,9 @@ struct flare_ctx {
     int max_ntn = 0;
     int ld = 0;
     double* d_accel = nullptr;  // [S] 0.5 dt kappa / m
+    double* d_mass = nullptr;   // [S] amu
+    bool last_eval_var = false; // the last evaluation produced variances (v_s is meaningful)
+    bool pairf_valid = false;   // an evaluation has been run since flare_bind (pair forces, neighbour list valid)
     double accel_dt = -1.0;
     std::vector<double> h_accel;
     // options
@@ -283,6 +286,9 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.W = cv.take<double>((size_t)chunk * c->ld);
     w.nrm = cv.take<double>(chunk);
     w.part = cv.take<double>((size_t)2 * std::max(c->max_ntn, 1) * chunk);
+    w.red = cv.take<double>((size_t)kRedBlocksMax * 9);
+    w.scal = cv.take<double>(16);
+    w.ascal = cv.take<unsigned long long>(18);
     if (ws) *ws = w;
     if (chunk_out) *chunk_out = chunk;
     if (cells_out) *cells_out = (int)std::min<size_t>(cells, 0x7fffffff);
@@ -366,6 +372,8 @@ int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, d
         run_gather(L, c->ws, n, c->mmax, e_out, f_out, var_out);
     }
     if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "launch");
+    c->last_eval_var = want_var;
+    c->pairf_valid = true;
     return FLARE_OK;
 }
 
@@ -431,6 +439,11 @@ int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_m
         void* d = nullptr;
         if (cudaMalloc(&d, sizeof(double) * kMaxSpecies) != cudaSuccess) rc = FLARE_ERR_CUDA;
         else { c->dev_allocs.push_back(d); c->d_accel = (double*)d; }
+    }
+    if (rc == FLARE_OK) {
+        std::vector<double> hm(kMaxSpecies, 1.0);
+        for (int s = 0; s < n_species; s++) hm[s] = mass_amu[s];
+        rc = upload(c, hm, &c->d_mass);
     }
     if (rc != FLARE_OK) { flare_destroy(c); return rc; }
     c->h_accel.assign(kMaxSpecies, 0.0);
@@ -506,7 +519,9 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     c->n = n_atoms;
     c->state_set = c->forces_valid = c->var_valid = false;
     c->have_grid = false;
+    c->pairf_valid = false;
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.flags, 0, sizeof(int) * 4, c->stream));
+    FLARE_CUDA(c, cudaMemsetAsync(c->ws.scal, 0, sizeof(double) * 16, c->stream));  // thermostat xi = eta = 0
     return FLARE_OK;
 }
 
@@ -602,7 +617,8 @@ static int set_forces_impl(flare_ctx* c, const double* f, cudaMemcpyKind kind) {
 int flare_set_forces(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyDeviceToDevice); }
 int flare_set_forces_host(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyHostToDevice); }
 
-int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
+// velocity Verlet; with T_kelvin > 0 each step is bracketed by Nose-Hoover half steps (R19)
+static int step_impl(flare_ctx* c, double dt_fs, int n_steps, int want_variance, double T_kelvin, double tau_fs) {
     int rc = need_bound(c);
     if (rc) return rc;
     if (!c->state_set) return fail(c, FLARE_ERR_NOT_BOUND, "flare_set_state has not been called");
@@ -630,9 +646,13 @@ int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
     Launcher L;
     L.stream = c->stream;
     L.launch_count = &c->launches;
+    const bool nvt = T_kelvin > 0.0;
+    const double gkT = (3.0 * (double)n - 3.0) * 8.617333262e-5 * T_kelvin;  // g k_B T, g = 3N - 3 (R13, R19)
+    const double Q = gkT * tau_fs * tau_fs;
     for (int step = 0; step < n_steps; step++) {
         {
             PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
+            if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
             run_kick_drift(L, c->grid, n, w.x, w.v, w.f, w.types, c->d_accel, dt_fs);
         }
         rc = evaluate(c, w.x, w.types, w.e, w.f, var);
@@ -640,10 +660,97 @@ int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
         {
             PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
             run_kick(L, n, w.v, w.f, w.types, c->d_accel);
+            if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
         }
     }
     c->var_valid = want_variance != 0;
     if (L.err != cudaSuccess) return cuda_fail(c, L.err, "integrator launch");
+    return FLARE_OK;
+}
+
+int flare_step(flare_ctx* c, double dt_fs, int n_steps, int want_variance) {
+    return step_impl(c, dt_fs, n_steps, want_variance, 0.0, 0.0);
+}
+
+int flare_step_nvt(flare_ctx* c, double dt_fs, int n_steps, int want_variance, double T_kelvin, double tau_fs) {
+    if (!c) return FLARE_ERR_INVALID_ARG;
+    if (!(T_kelvin > 0.0) || !(tau_fs > 0.0) || !std::isfinite(T_kelvin) || !std::isfinite(tau_fs))
+        return fail(c, FLARE_ERR_INVALID_ARG, "thermostat temperature and time constant must be > 0");
+    if (c->n >= 0 && c->n < 2) return fail(c, FLARE_ERR_INVALID_ARG, "the thermostat needs at least 2 atoms (g = 3N - 3)");
+    return step_impl(c, dt_fs, n_steps, want_variance, T_kelvin, tau_fs);
+}
+
+int flare_get_thermostat(flare_ctx* c, double* xi, double* eta) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    double h[2] = {0.0, 0.0};
+    FLARE_CUDA(c, cudaMemcpy(h, c->ws.scal + 12, sizeof(h), cudaMemcpyDeviceToHost));
+    if (xi) *xi = h[0];
+    if (eta) *eta = h[1];
+    return FLARE_OK;
+}
+
+int flare_set_thermostat(flare_ctx* c, double xi, double eta) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!std::isfinite(xi) || !std::isfinite(eta)) return fail(c, FLARE_ERR_INVALID_ARG, "non-finite thermostat state");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    const double h[2] = {xi, eta};
+    FLARE_CUDA(c, cudaMemcpy(c->ws.scal + 12, h, sizeof(h), cudaMemcpyHostToDevice));
+    return FLARE_OK;
+}
+
+int flare_get_virial(flare_ctx* c, double virial[9]) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!virial) return fail(c, FLARE_ERR_INVALID_ARG, "virial is null");
+    if (!c->pairf_valid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    for (int q = 0; q < 9; q++) virial[q] = 0.0;
+    if (c->n == 0) return FLARE_OK;
+    Launcher L;
+    L.stream = c->stream;
+    L.launch_count = &c->launches;
+    run_virial(L, c->grid, c->ws, (int)c->n, c->mmax, c->ws.scal);
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, "virial launch");
+    FLARE_CUDA(c, cudaMemcpyAsync(virial, c->ws.scal, sizeof(double) * 9, cudaMemcpyDeviceToHost, c->stream));
+    return flare_check(c);
+}
+
+int flare_analyze(flare_ctx* c, double unc_threshold, int species_a, int species_b, double r_coord, double* max_unc,
+                  int64_t* n_above, int32_t* coord, int64_t* coord_hist) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->pairf_valid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    const bool want_unc = max_unc || n_above;
+    const bool want_coord = coord || coord_hist;
+    if (want_unc && !c->last_eval_var) return fail(c, FLARE_ERR_INVALID_ARG, "the last evaluation had no variances");
+    if (want_coord) {
+        if (species_a < 0 || species_a >= c->bs.S || species_b < 0 || species_b >= c->bs.S)
+            return fail(c, FLARE_ERR_INVALID_ARG, "species out of range");
+        // the neighbour list only holds pairs inside r_cut[a][b]
+        if (!(r_coord > 0.0) || r_coord > c->bs.rc[species_a * c->bs.S + species_b])
+            return fail(c, FLARE_ERR_INVALID_ARG, "r_coord must be in (0, r_cut[a][b]]");
+    }
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    unsigned long long h[18] = {0};
+    if (c->n > 0 && (want_unc || want_coord)) {
+        Launcher L;
+        L.stream = c->stream;
+        L.launch_count = &c->launches;
+        run_analyze(L, c->grid, c->ws, (int)c->n, c->mmax, want_unc, unc_threshold, species_a, species_b, r_coord,
+                    want_coord, coord, c->ws.ascal);
+        if (L.err != cudaSuccess) return cuda_fail(c, L.err, "analysis launch");
+        FLARE_CUDA(c, cudaMemcpyAsync(h, c->ws.ascal, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    }
+    rc = flare_check(c);
+    if (rc) return rc;
+    if (max_unc) { double u; memcpy(&u, &h[0], sizeof(u)); *max_unc = u; }
+    if (n_above) *n_above = (int64_t)h[1];
+    if (coord_hist) for (int q = 0; q < 16; q++) coord_hist[q] = (int64_t)h[2 + q];
     return FLARE_OK;
 }
 

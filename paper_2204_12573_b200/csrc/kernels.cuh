@@ -70,7 +70,12 @@ struct Workspace {
     double* W = nullptr;     // [chunk][Pld]
     double* nrm = nullptr;   // [chunk]
     double* part = nullptr;  // [2][max_ntn][chunk]  partial row-dots of the energy / variance tiles
+    // ---- reductions and scalars of the analysis / thermostat kernels
+    double* red = nullptr;                 // [kRedBlocksMax][9] per-block partial sums
+    double* scal = nullptr;                // [16]: [0..8] virial, [12..15] thermostat xi, eta, scale, K2
+    unsigned long long* ascal = nullptr;   // [18] analysis outputs (max bits, count, coordination histogram)
 };
+constexpr int kRedBlocksMax = 1184;
 
 // One quadratic-form group: rows whose atoms share the matrix (and, in sparse mode, the component set).
 struct GroupDesc {
@@ -135,6 +140,14 @@ void run_gather(Launcher& L, const Workspace& ws, int n, int mmax, double* e_out
 void run_kick_drift(Launcher& L, const Grid& g, int n, double* x, double* v, const double* f, const int* types,
                     const double* accel_half_dt /*[S] device: 0.5 dt kappa / m*/, double dt);
 void run_kick(Launcher& L, int n, double* v, const double* f, const int* types, const double* accel_half_dt);
+
+// analysis.cu: virial -> out9 (device), analysis -> out18 (device), one Nose-Hoover half step of length h
+void run_virial(Launcher& L, const Grid& g, const Workspace& ws, int n, int mmax, double* out9);
+void run_analyze(Launcher& L, const Grid& g, const Workspace& ws, int n, int mmax, bool have_var, double threshold,
+                 int species_a, int species_b, double r_coord, bool want_coord, int* coord,
+                 unsigned long long* out18);
+void run_nh_half(Launcher& L, const Workspace& ws, int n, const double* mass_dev, double h, double gkT, double Q,
+                 double* thermo);
 
 double measure_dmma_peak(int device);
 

@@ -31,6 +31,7 @@ EXPORTS = (
     "flare_set_state", "flare_set_state_host", "flare_set_forces", "flare_set_forces_host", "flare_step", "flare_get_state", "flare_get_state_host",
     "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_timings", "flare_kernel_launches",
     "flare_measure_fp64_dmma_peak", "flare_last_error",
+    "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_analyze",
 )
 
 
@@ -82,6 +83,11 @@ def load_library():
     lib.flare_measure_fp64_dmma_peak.restype = dbl
     lib.flare_last_error.argtypes = [vp]
     lib.flare_last_error.restype = C.c_char_p
+    lib.flare_step_nvt.argtypes = [vp, dbl, i32, i32, dbl, dbl]
+    lib.flare_get_thermostat.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.flare_set_thermostat.argtypes = [vp, dbl, dbl]
+    lib.flare_get_virial.argtypes = [vp, vp]
+    lib.flare_analyze.argtypes = [vp, dbl, i32, i32, dbl, C.POINTER(dbl), C.POINTER(i64), vp, vp]
     _lib = lib
     return lib
 
@@ -259,6 +265,37 @@ class Flare:
 
     def step(self, dt_fs: float, n_steps: int = 1, want_variance: bool = False):
         self._check(self._lib.flare_step(self._ctx, float(dt_fs), int(n_steps), 1 if want_variance else 0))
+
+    def step_nvt(self, dt_fs: float, n_steps: int, T_kelvin: float, tau_fs: float, want_variance: bool = False):
+        self._check(self._lib.flare_step_nvt(self._ctx, float(dt_fs), int(n_steps), 1 if want_variance else 0,
+                                             float(T_kelvin), float(tau_fs)))
+
+    def thermostat(self):
+        xi, eta = C.c_double(0.0), C.c_double(0.0)
+        self._check(self._lib.flare_get_thermostat(self._ctx, C.byref(xi), C.byref(eta)))
+        return xi.value, eta.value
+
+    def set_thermostat(self, xi: float, eta: float):
+        self._check(self._lib.flare_set_thermostat(self._ctx, float(xi), float(eta)))
+
+    def virial(self):
+        """[3,3] virial dE/d eps (eV) of the last evaluation."""
+        w = np.zeros(9)
+        self._check(self._lib.flare_get_virial(self._ctx, _hp(w)))
+        return w.reshape(3, 3)
+
+    def analyze(self, threshold: float = 0.0, species_a: int = 0, species_b: int = 0, r_coord: float = 1.0,
+                uncertainty: bool = True, coordination: bool = True):
+        """dict(max_unc, n_above, coord (device int32 tensor), hist[16]) of the last evaluation."""
+        mx, na = C.c_double(0.0), C.c_int64(0)
+        hist = np.zeros(16, np.int64)
+        coord = self._torch.zeros(self.n_atoms, dtype=self._torch.int32, device=self.device) if coordination else None
+        self._check(self._lib.flare_analyze(
+            self._ctx, float(threshold), int(species_a), int(species_b), float(r_coord),
+            C.byref(mx) if uncertainty else None, C.byref(na) if uncertainty else None,
+            C.c_void_p(coord.data_ptr()) if coordination else None, _hp(hist) if coordination else None))
+        return dict(max_unc=mx.value if uncertainty else None, n_above=na.value if uncertainty else None,
+                    coord=coord, hist=hist if coordination else None)
 
     def get_state(self, variances: bool = False):
         """Device tensors dict(pos, vel, E, F[, V])."""
