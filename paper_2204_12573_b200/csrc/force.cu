@@ -90,7 +90,7 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gs_ = max(group_start[gr.g], gr.row0);
     const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
-    const int r0 = (blockIdx.x * kBpWarps + warp) * ta;
+    const int r0 = (blockIdx.x * (blockDim.x >> 5) + warp) * ta;  // 1..kBpWarps warps per CTA (shared-memory budget)
     if (r0 >= ge_ - gs_) return;  // warps are independent: only __syncwarp below
     const int na = min(ta, ge_ - gs_ - r0);
     const int lrow0 = gs_ - gr.row0 + r0;
@@ -295,14 +295,22 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
         ta = budget / (gr.nsp * SM::GB);
         ta = ta < 1 ? 1 : (ta > kBpMaxTA ? kBpMaxTA : ta);
     }
-    const size_t smem = sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
+    // warps per CTA: as many of kBpWarps as fit the 227 KB of shared memory a CTA can have (large (n_max, l_max))
+    const size_t per_warp = sizeof(double) * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
+    int warps = kBpWarps;
+    while (warps > 1 && per_warp * warps > 220 * 1024) warps--;
+    const size_t smem = per_warp * warps;
+    if (smem > 227 * 1024) {
+        if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.err_where = "back-propagation: descriptor too large for shared memory"; }
+        return;
+    }
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
         cudaFuncSetAttribute(k_backprop<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    const int per_cta = kBpWarps * ta;
-    L.launch(k_backprop<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(kBpWarps * 32), smem, g, bs, yn, gr,
+    const int per_cta = warps * ta;
+    L.launch(k_backprop<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(warps * 32), smem, g, bs, yn, gr,
              ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const int*)ws.group_start, (const double*)ws.A, (const double*)ws.Bh,
              (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap, max_ntn,

@@ -97,7 +97,7 @@ def test_config2_full(oracle, torch, flare, sparse):
 
 
 @pytest.mark.parametrize("sparse", [True, False])
-@pytest.mark.parametrize("n_max,l_max", [(1, 0), (3, 1), (4, 2), (7, 3), (3, 4), (2, 5), (2, 6), (5, 6), (9, 2)])
+@pytest.mark.parametrize("n_max,l_max", [(1, 0), (3, 1), (4, 2), (7, 3), (3, 4), (2, 5), (2, 6), (5, 6), (9, 2), (10, 4), (12, 6), (16, 1)])
 def test_basis_sizes_on_a_small_tile(oracle, torch, flare, n_max, l_max, sparse):
     s = w.tile_like_c3(6, 3, n_max=n_max, l_max=l_max)  # 216 Pt + 18 H
     assert_parity(oracle, torch, flare, s, species_sparse=sparse)
