@@ -159,6 +159,72 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------- GPU arm, decomposed (opt-in)
+
+
+def run_decomposed(args):
+    """Weak scaling of the real multi-GPU path: one H2/Pt(111) slab `world` times as long as C3 along x, cut into
+    `world` slabs, halo exchange every step (NCCL point-to-point).  Same JSON line; roofline / cpu_baseline omitted."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2204_12573_b200 import flare
+    from paper_2204_12573_b200.halo import CudaEngine, SlabDecomposition
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    want_var = not args.no_variance
+    s = workloads.h2_pt111_config(3, 408 * world, 204, 41616 * world, name=f"C3x{world}")
+    ctx = flare.from_system(s, device=local, variance=want_var)
+    eng = CudaEngine(ctx, capacity=int(1.2 * s.n_atoms / world) + 4096)
+    dd = SlabDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), axis=0).scatter(s.pos, s.vel, s.types)
+    dt_fs = float(s.meta.get("dt_fs", 0.5))
+    dd.compute(want_var)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dd.step(dt_fs, args.warmup, want_var)
+    launches0 = ctx.kernel_launches()
+    sent0 = dd.bytes_sent
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    dd.step(dt_fs, args.steps, want_var)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else {}
+    ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=torch.device("cuda", local))
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": s.n_atoms * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"C3 construction {world}x as long along x: {s.n_atoms} atoms on {world} slab(s), "
+                                   "halo 2 r_cut, one exchange + one migration per step", "atoms": s.n_atoms, "P": s.P,
+                       "variance": want_var, "dt_fs": dt_fs, "parallelism": f"slab decomposition x{world}",
+                       "halo_bytes_per_rank_per_step": (dd.bytes_sent - sent0) / max(1, args.steps),
+                       "l2": "working set far larger than L2; no flush needed"},
+            "clocks": clocks, "gpu_launches": ctx.kernel_launches() - launches0,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 # ----------------------------------------------------------------------------- GPU arm
 
 
@@ -333,10 +399,15 @@ def main():
     ap.add_argument("--no-variance", action="store_true")
     ap.add_argument("--dense", action="store_true", help="switch the species-sparse evaluation (P:L155) off")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomposed", action="store_true",
+                    help="N ranks share ONE system N times as long as C3 (slab decomposition + halo exchange, "
+                         "paper_2204_12573_b200/halo.py) instead of running N replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomposed:
+        run_decomposed(args)
     else:
         run_ours(args)
 

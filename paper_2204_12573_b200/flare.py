@@ -182,16 +182,20 @@ class Flare:
     def workspace_bytes(self, n_atoms: int) -> int:
         return int(self._lib.flare_workspace_bytes(self._ctx, int(n_atoms)))
 
-    def bind(self, n_atoms: int, stream=None):
-        """Allocate (torch) and attach the workspace for n_atoms on `stream` (default: current)."""
+    def bind(self, n_atoms: int, stream=None, workspace=None):
+        """Attach the workspace for n_atoms on `stream` (default: current).  The workspace is a torch uint8 tensor:
+        allocated here, or an earlier (large enough) one passed as `workspace` to avoid re-allocation."""
         torch = self._torch
         nbytes = self.workspace_bytes(n_atoms)
         if nbytes == 0:
             raise FlareError(-1, "flare_workspace_bytes returned 0")
-        self._workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        if workspace is not None and workspace.numel() >= nbytes:
+            self._workspace = workspace
+        else:
+            self._workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self._check(self._lib.flare_bind(self._ctx, int(n_atoms), C.c_void_p(self._workspace.data_ptr()), nbytes,
-                                         C.c_void_p(self._stream.cuda_stream)))
+        self._check(self._lib.flare_bind(self._ctx, int(n_atoms), C.c_void_p(self._workspace.data_ptr()),
+                                         self._workspace.numel(), C.c_void_p(self._stream.cuda_stream)))
         self.n_atoms = int(n_atoms)
         return self
 
