@@ -269,6 +269,68 @@ k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int*
     }
 }
 
+// Thread per atom (the default for mmax <= 64).  A CTA takes 128 consecutive cell-sorted atoms; every thread walks the
+// (up to 18) candidate runs of its own cell neighbourhood, testing one candidate per iteration.  Threads of a warp sit
+// in the same or adjacent cells, so their candidate loads hit the same few 32-byte sectors (L1 broadcast), and the
+// per-candidate cost is the ~20 instructions of the canonical distance test instead of a warp-wide sweep with shuffles.
+// Hits are staged in shared memory (one padded row per thread) and copied out as coalesced rows.
+constexpr int kNbrThreads = 128;
+
+__global__ void __launch_bounds__(kNbrThreads)
+k_neighbors_tpa(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int* __restrict__ cell_start, int mmax,
+                int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx, unsigned char* __restrict__ nmask,
+                int* __restrict__ flags) {
+    extern __shared__ int stage[];  // [kNbrThreads][mmax | 1]
+    const int ST = mmax | 1;
+    const int k = blockIdx.x * kNbrThreads + threadIdx.x;
+    int cnt = 0;
+    unsigned mask = 0;
+    if (k < n) {
+        const AtomS me = load_atom(atoms + k);
+        int c[3];
+        c[0] = max(0, min(g.nc[0] - 1, (int)floor(me.x * g.inv_cw[0])));
+        c[1] = max(0, min(g.nc[1] - 1, (int)floor(me.y * g.inv_cw[1])));
+        c[2] = max(0, min(g.nc[2] - 1, (int)floor(me.z * g.inv_cw[2])));
+        int ca[3], cb[3], flo[2], fhi[2];
+        const int na = slow_cells(g, g.slow0, c[g.slow0], ca);
+        const int nb = slow_cells(g, g.slow1, c[g.slow1], cb);
+        const int nf = fast_ranges(g, c[g.fast], flo, fhi);
+        const double* rc2 = bs.rc2 + me.type * bs.S;
+        int* row = stage + threadIdx.x * ST;
+        for (int ib = 0; ib < nb; ib++)
+            for (int ia = 0; ia < na; ia++) {
+                const int base = ca[ia] * g.stride[g.slow0] + cb[ib] * g.stride[g.slow1];
+                for (int r = 0; r < nf; r++) {
+                    const int qs = __ldg(cell_start + base + flo[r]);
+                    const int qe = __ldg(cell_start + base + fhi[r] + 1);
+                    for (int q = qs; q < qe; q++) {
+                        if (q == k) continue;
+                        const AtomS o = load_atom(atoms + q);
+                        double dx, dy, dz;
+                        displacement(g, me, o, dx, dy, dz);
+                        if (dist2_canonical(dx, dy, dz) < rc2[o.type]) {  // strict (R6)
+                            if (cnt < mmax) row[cnt] = q;
+                            cnt++;
+                            mask |= 1u << o.type;
+                        }
+                    }
+                }
+            }
+        if (cnt > mmax) { atomicOr(flags, kFlagNeighborOverflow); cnt = mmax; }
+        nbr_cnt[k] = cnt;
+        nmask[k] = (unsigned char)mask;
+    }
+    // coalesced copy-out: each warp writes the rows of its own 32 threads, one row at a time
+    __syncwarp();
+    const int lane = threadIdx.x & 31, w0 = threadIdx.x & ~31;
+    for (int t = 0; t < 32; t++) {
+        const int ct = __shfl_sync(kFull, cnt, t);
+        const int kt = blockIdx.x * kNbrThreads + w0 + t;
+        const int* src = stage + (w0 + t) * ST;
+        for (int s = lane; s < ct; s += 32) nbr_idx[(size_t)kt * mmax + s] = src[s];
+    }
+}
+
 // rev[k][s] = slot of k in the row of j = nbr_idx[k][s]  (exists because cutoffs are symmetric, R5).
 // Lane s holds neighbour s and its row length; the rows of four neighbours are fetched together (one
 // coalesced 128-byte read each) before any of them is searched, and the found slots are written back as
@@ -399,8 +461,14 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
     L.launch(k_sort_cells, dim3((g.n_cells + tb - 1) / tb), dim3(tb), 0, g.n_cells, (const int*)ws.cell_start, ws.order);
     L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order, ws.atoms);
     const int nwb = (n + kNbrWarps - 1) / kNbrWarps;
-    L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bs, n, (const AtomS*)ws.atoms,
-             (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+    if (mmax <= 64) {
+        const size_t stage = sizeof(int) * kNbrThreads * (size_t)(mmax | 1);
+        L.launch(k_neighbors_tpa, dim3((n + kNbrThreads - 1) / kNbrThreads), dim3(kNbrThreads), stage, g, bs, n,
+                 (const AtomS*)ws.atoms, (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+    } else {
+        L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bs, n, (const AtomS*)ws.atoms,
+                 (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+    }
     L.launch(k_reverse_index, dim3(nwb), dim3(kNbrWarps * 32), 0, n, mmax, (const int*)ws.nbr_cnt,
              (const int*)ws.nbr_idx, ws.rev);
     const int ngb = (n + kGroupBlock - 1) / kGroupBlock;
