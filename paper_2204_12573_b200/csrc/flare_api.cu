@@ -49,6 +49,8 @@ struct flare_ctx {
     int ld = 0;
     double* d_accel = nullptr;  // [S] 0.5 dt kappa / m
     double* d_mass = nullptr;   // [S] amu
+    double skin = 0.4;          // Angstrom; 0 = rebuild the neighbour list at every evaluation
+    bool list_valid = false;    // a skin list exists for the bound workspace and the current grid
     bool last_eval_var = false; // the last evaluation produced variances (v_s is meaningful)
     bool pairf_valid = false;   // an evaluation has been run since flare_bind (pair forces, neighbour list valid)
     double accel_dt = -1.0;
@@ -120,6 +122,9 @@ struct PhaseScope {
 };
 
 int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// the skin list needs one 64-bit hit mask per atom: rows longer than 64 switch it off
+double eff_skin(const flare_ctx* c) { return c->mmax <= kSkinStride ? c->skin : 0.0; }
 
 // choose the tile width (in n8 blocks) that wastes the fewest padded columns; ties -> wider tile
 void choose_tiles(int K, int& nb, int& ntn) {
@@ -278,6 +283,14 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.row_of = cv.take<int>(N);
     w.gid = cv.take<unsigned char>(N);
     w.atom_of_row = cv.take<int>(N);
+    if (eff_skin(c) > 0.0) {
+        w.skin_cnt = cv.take<int>(N);
+        w.skin_idx = cv.take<int>(N * kSkinStride);
+        w.skin_rev = cv.take<unsigned char>(N * kSkinStride);
+        w.ref = cv.take<AtomS>(N);
+        w.hitmask = cv.take<unsigned long long>(N);
+        w.skin_gate = cv.take<int>(4);
+    }
     w.pairf = cv.take<double>(N * c->mmax * 3);
     w.e_s = cv.take<double>(N);
     w.v_s = cv.take<double>(N);
@@ -312,7 +325,7 @@ int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
         g.pbc[d] = pbc[d] ? 1 : 0;
         if (g.pbc[d] && g.L[d] < 2.0 * rcmax)
             return fail(c, FLARE_ERR_BOX_TOO_SMALL, "a periodic box length is < 2 max r_cut (R7)");
-        int nc = (int)std::floor(g.L[d] / (rcmax * (1.0 + 1e-9)));
+        int nc = (int)std::floor(g.L[d] / ((rcmax + eff_skin(c)) * (1.0 + 1e-9)));  // cells hold the skin list's cutoff
         g.nc[d] = std::max(1, nc);
     }
     // keep the number of cells within what the workspace was sized for
@@ -330,6 +343,7 @@ int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
     g.stride[g.slow0] = g.nc[g.fast];
     g.stride[g.slow1] = g.nc[g.fast] * g.nc[g.slow0];
     g.n_cells = g.nc[0] * g.nc[1] * g.nc[2];
+    if (!c->have_grid || memcmp(&c->grid, &g, sizeof(Grid)) != 0) c->list_valid = false;  // new box: new list
     c->grid = g;
     c->have_grid = true;
     memcpy(c->box, box, sizeof(double) * 9);
@@ -348,7 +362,9 @@ int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, d
     if (n == 0) return FLARE_OK;
     {
         PhaseScope ps(c, FLARE_PHASE_NEIGHBOR);
-        build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups);
+        build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups, eff_skin(c),
+                        c->list_valid);
+        if (eff_skin(c) > 0.0) c->list_valid = true;
     }
     for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
         const int nrows = std::min(c->chunk_cap, n - row0);
@@ -478,6 +494,10 @@ int flare_set_option(flare_ctx* c, int option, int64_t value) {
         case FLARE_OPT_TIMING:
             c->timing = value ? 1 : 0;
             return FLARE_OK;
+        case FLARE_OPT_SKIN_MILLI_ANGSTROM:
+            if (value < 0 || value > 4000) return fail(c, FLARE_ERR_INVALID_ARG, "skin must be in 0..4000 (1e-3 Angstrom)");
+            c->skin = 1e-3 * (double)value; c->n = -1;
+            return FLARE_OK;
         case FLARE_OPT_SPECIES_SPARSE:
             if (value && !c->have_sparse)
                 return fail(c, FLARE_ERR_UNSUPPORTED, "species-sparse mode needs S * 2^S <= 64 groups");
@@ -496,6 +516,18 @@ int flare_get_option(const flare_ctx* c, int option, int64_t* value) {
         case FLARE_OPT_CHUNK_ATOMS: *value = c->n >= 0 ? c->chunk_cap : c->chunk_opt; return FLARE_OK;
         case FLARE_OPT_TIMING: *value = c->timing; return FLARE_OK;
         case FLARE_OPT_SPECIES_SPARSE: *value = c->sparse; return FLARE_OK;
+        case FLARE_OPT_SKIN_MILLI_ANGSTROM: *value = (int64_t)std::llround(c->skin * 1e3); return FLARE_OK;
+        case FLARE_OPT_SKIN_REBUILDS: {
+            *value = 0;
+            if (c->n >= 0 && c->ws.skin_gate) {
+                int h = 0;
+                if (cudaStreamSynchronize(c->stream) != cudaSuccess ||
+                    cudaMemcpy(&h, c->ws.skin_gate + 1, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)
+                    return FLARE_ERR_CUDA;
+                *value = h;
+            }
+            return FLARE_OK;
+        }
         default: return FLARE_ERR_INVALID_ARG;
     }
 }
@@ -520,8 +552,10 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     c->state_set = c->forces_valid = c->var_valid = false;
     c->have_grid = false;
     c->pairf_valid = false;
+    c->list_valid = false;
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.flags, 0, sizeof(int) * 4, c->stream));
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.scal, 0, sizeof(double) * 16, c->stream));  // thermostat xi = eta = 0
+    if (c->ws.skin_gate) FLARE_CUDA(c, cudaMemsetAsync(c->ws.skin_gate, 0, sizeof(int) * 4, c->stream));
     return FLARE_OK;
 }
 
@@ -545,7 +579,7 @@ int flare_check(flare_ctx* c) {
     if (flags[0]) FLARE_CUDA(c, cudaMemset(c->ws.flags, 0, sizeof(flags)));
     if (flags[0] & kFlagNonFinite) return fail(c, FLARE_ERR_NONFINITE, "non-finite position");
     if (flags[0] & kFlagNeighborOverflow)
-        return fail(c, FLARE_ERR_NEIGHBOR_OVERFLOW, "an atom has more neighbours than FLARE_OPT_MAX_NEIGHBORS");
+        return fail(c, FLARE_ERR_NEIGHBOR_OVERFLOW, "an atom has more neighbours than FLARE_OPT_MAX_NEIGHBORS (or more than 64 candidates within r_cut + skin: lower FLARE_OPT_SKIN_MILLI_ANGSTROM)");
     return FLARE_OK;
 }
 

@@ -10,6 +10,7 @@ namespace flare {
 
 constexpr int kMaxGroups = 64;  // quadratic-form groups: (central species) or (species, neighbour mask)
 constexpr int kNumPhases = 6;
+constexpr int kSkinStride = 64;  // row stride of the skin (candidate) list: one 64-bit hit mask per atom
 
 // Launch wrapper: all kernels go to one stream; counts launches; keeps the first CUDA error.
 struct Launcher {
@@ -60,6 +61,13 @@ struct Workspace {
     int* row_of = nullptr;        // [N] sorted atom -> quadratic-form row
     unsigned char* gid = nullptr; // [N] group id of each sorted atom
     int* atom_of_row = nullptr;   // [N]
+    // ---- skin list (candidates within r_cut + skin, kept across evaluations; only with FLARE_OPT_SKIN > 0)
+    int* skin_cnt = nullptr;               // [N]
+    int* skin_idx = nullptr;               // [N][kSkinStride]
+    unsigned char* skin_rev = nullptr;     // [N][kSkinStride] reverse index of the candidate list
+    AtomS* ref = nullptr;                  // [N] sorted atoms at the time the list was built
+    unsigned long long* hitmask = nullptr; // [N] bit s: candidate s passes the exact predicate
+    int* skin_gate = nullptr;              // [1] non-zero: rebuild in this evaluation
     // ---- per-atom results in sorted order
     double* pairf = nullptr;  // [N][mmax][3]  dE_k/dr_kj
     double* e_s = nullptr;    // [N]
@@ -119,8 +127,10 @@ struct GroupDev {
 };
 
 // stage entry points (each enqueues kernels through the Launcher)
+// skin > 0: keep a candidate list with cutoffs r_cut + skin across evaluations (list_valid: one exists for this
+// order / box / types) and filter it with the exact predicate; skin = 0: rebuild everything every time.
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
-                     const int* types, int mmax, int sparse, int n_groups);
+                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid);
 
 // Descriptor rows [row0,row0+nrows): compact A -> ws.A, UNNORMALISED B -> bh_out (row r at (r - row0)*ld),
 // ||B|| -> nrm_out.  One launch per group.

@@ -8,7 +8,8 @@ namespace flare {
 
 // ------------------------------------------------------------------ wrap + cell assignment
 __global__ void k_cell_assign(Grid g, int n, const double* __restrict__ pos, int* __restrict__ cell_of,
-                              int* __restrict__ rank_in_cell, int* __restrict__ cell_cnt, int* __restrict__ flags) {
+                              int* __restrict__ rank_in_cell, int* __restrict__ cell_cnt, int* __restrict__ flags, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double p[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
@@ -30,7 +31,8 @@ __global__ void k_cell_assign(Grid g, int n, const double* __restrict__ pos, int
 // ------------------------------------------------------------------ exclusive scan (3 launches)
 constexpr int kScanBlock = 1024;
 
-__global__ void k_scan_partial(int n, const int* __restrict__ in, int* __restrict__ out, int* __restrict__ block_sum) {
+__global__ void k_scan_partial(int n, const int* __restrict__ in, int* __restrict__ out, int* __restrict__ block_sum, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     __shared__ int warp_tot[32];
     int i = blockIdx.x * kScanBlock + threadIdx.x;
     int v = (i < n) ? in[i] : 0;
@@ -59,7 +61,8 @@ __global__ void k_scan_partial(int n, const int* __restrict__ in, int* __restric
 }
 
 // single block: exclusive scan of the block sums in place
-__global__ void k_scan_sums(int nb, int* __restrict__ block_sum) {
+__global__ void k_scan_sums(int nb, int* __restrict__ block_sum, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     __shared__ int carry_s;
     __shared__ int warp_tot[32];
     if (threadIdx.x == 0) carry_s = 0;
@@ -95,29 +98,32 @@ __global__ void k_scan_sums(int nb, int* __restrict__ block_sum) {
     }
 }
 
-__global__ void k_scan_add(int n, int* __restrict__ out, const int* __restrict__ block_sum) {
+__global__ void k_scan_add(int n, int* __restrict__ out, const int* __restrict__ block_sum, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int i = blockIdx.x * kScanBlock + threadIdx.x;
     if (i < n) out[i] += block_sum[blockIdx.x];
 }
 
 // out[n] = out[n-1] + in[n-1]
-__global__ void k_scan_total(int n, const int* __restrict__ in, int* __restrict__ out) {
+__global__ void k_scan_total(int n, const int* __restrict__ in, int* __restrict__ out, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     if (threadIdx.x == 0 && blockIdx.x == 0) out[n] = (n > 0) ? out[n - 1] + in[n - 1] : 0;
 }
 
-void exclusive_scan(Launcher& L, int n, const int* in, int* out /*[n+1]*/, int* block_sum) {
+void exclusive_scan(Launcher& L, int n, const int* in, int* out /*[n+1]*/, int* block_sum, const int* gate) {
     int nb = (n + kScanBlock - 1) / kScanBlock;
     if (n > 0) {
-        L.launch(k_scan_partial, dim3(nb), dim3(kScanBlock), 0, n, in, out, block_sum);
-        L.launch(k_scan_sums, dim3(1), dim3(kScanBlock), 0, nb, block_sum);
-        L.launch(k_scan_add, dim3(nb), dim3(kScanBlock), 0, n, out, (const int*)block_sum);
+        L.launch(k_scan_partial, dim3(nb), dim3(kScanBlock), 0, n, in, out, block_sum, gate);
+        L.launch(k_scan_sums, dim3(1), dim3(kScanBlock), 0, nb, block_sum, gate);
+        L.launch(k_scan_add, dim3(nb), dim3(kScanBlock), 0, n, out, (const int*)block_sum, gate);
     }
-    L.launch(k_scan_total, dim3(1), dim3(32), 0, n, in, out);
+    L.launch(k_scan_total, dim3(1), dim3(32), 0, n, in, out, gate);
 }
 
 // ------------------------------------------------------------------ counting sort by cell
 __global__ void k_scatter(int n, const int* __restrict__ cell_of, const int* __restrict__ rank_in_cell,
-                          const int* __restrict__ cell_start, int* __restrict__ order) {
+                          const int* __restrict__ cell_start, int* __restrict__ order, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     order[cell_start[cell_of[i]] + rank_in_cell[i]] = i;
@@ -125,7 +131,8 @@ __global__ void k_scatter(int n, const int* __restrict__ cell_of, const int* __r
 
 // The arrival order of atomicAdd inside a cell is not reproducible: sort each cell's (few) atoms by
 // their index in the caller's order so that the whole pipeline is run-to-run deterministic.
-__global__ void k_sort_cells(int n_cells, const int* __restrict__ cell_start, int* __restrict__ order) {
+__global__ void k_sort_cells(int n_cells, const int* __restrict__ cell_start, int* __restrict__ order, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_cells) return;
     int s = cell_start[c], e = cell_start[c + 1];
@@ -138,7 +145,8 @@ __global__ void k_sort_cells(int n_cells, const int* __restrict__ cell_start, in
 }
 
 __global__ void k_gather_atoms(Grid g, int n, const double* __restrict__ pos, const int* __restrict__ types,
-                               const int* __restrict__ order, AtomS* __restrict__ atoms) {
+                               const int* __restrict__ order, AtomS* __restrict__ atoms, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     int i = order[k];
@@ -197,7 +205,8 @@ constexpr int kNbrWarps = 8;
 __global__ void __launch_bounds__(kNbrWarps * 32)
 k_neighbors(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int* __restrict__ cell_start, int mmax,
             int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx, unsigned char* __restrict__ nmask,
-            int* __restrict__ flags) {
+            int* __restrict__ flags, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     const int lane = threadIdx.x & 31;
     const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
     if (k >= n) return;
@@ -279,7 +288,8 @@ constexpr int kNbrThreads = 128;
 __global__ void __launch_bounds__(kNbrThreads)
 k_neighbors_tpa(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const int* __restrict__ cell_start, int mmax,
                 int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx, unsigned char* __restrict__ nmask,
-                int* __restrict__ flags) {
+                int* __restrict__ flags, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     extern __shared__ int stage[];  // [kNbrThreads][mmax | 1]
     const int ST = mmax | 1;
     const int k = blockIdx.x * kNbrThreads + threadIdx.x;
@@ -337,7 +347,8 @@ k_neighbors_tpa(Grid g, Basis bs, int n, const AtomS* __restrict__ atoms, const 
 // one coalesced byte store per 32 neighbours.
 __global__ void __launch_bounds__(kNbrWarps * 32)
 k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx,
-                unsigned char* __restrict__ rev) {
+                unsigned char* __restrict__ rev, const int* __restrict__ gate) {
+    if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     const int lane = threadIdx.x & 31;
     const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
     if (k >= n) return;
@@ -369,6 +380,151 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
             }
         }
         if (s < cnt) rev[(size_t)k * mmax + s] = (unsigned char)mine;
+    }
+}
+
+// ------------------------------------------------------------------ skin list (R12: "a skin list filtered by the exact
+// predicate is allowed, sets must still be exact").  Between rebuilds the cell-sorted order and a candidate list built
+// with cutoffs r_cut + skin are kept; every evaluation refreshes the sorted positions, checks that no atom has moved
+// further than skin/2 from where it was when the list was built (else the gate is raised and the whole build chain
+// above runs again), and filters the candidates with the exact canonical predicate.  The reverse-pair index of the
+// filtered list follows from the candidate list's own reverse index and the per-atom hit masks, without any search.
+
+// sorted positions <- current positions (in the order of the last build); raise the gate if anyone moved too far
+__global__ void k_refresh(Grid g, int n, const double* __restrict__ pos, const int* __restrict__ types,
+                          const int* __restrict__ order, const AtomS* __restrict__ ref, double half_skin2,
+                          AtomS* __restrict__ atoms, int* __restrict__ gate, int* __restrict__ flags) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int i = order[k];
+    double p[3] = {pos[3 * (size_t)i], pos[3 * (size_t)i + 1], pos[3 * (size_t)i + 2]};
+    bool bad = false;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        if (!isfinite(p[d])) { bad = true; p[d] = 0.0; }
+        if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
+    }
+    AtomS a;
+    a.x = p[0]; a.y = p[1]; a.z = p[2];
+    a.type = types[i];
+    a.orig = i;
+    atoms[k] = a;
+    const AtomS r = load_atom(ref + k);
+    double dx, dy, dz;
+    displacement(g, r, a, dx, dy, dz);
+    const bool moved = bad || !(dx * dx + dy * dy + dz * dz < half_skin2) || r.type != a.type;
+    if (bad) atomicOr(flags, kFlagNonFinite);
+    if (moved) *gate = 1;  // benign race: every writer stores 1
+}
+
+__global__ void k_copy_ref(int n, const AtomS* __restrict__ atoms, AtomS* __restrict__ ref, const int* __restrict__ gate,
+                           int* __restrict__ n_rebuilds) {
+    if (gate != nullptr && *gate == 0) return;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) ref[k] = atoms[k];
+    if (k == 0) *n_rebuilds += 1;  // statistics (FLARE_OPT_SKIN_REBUILDS)
+}
+
+// A warp takes kFilterAtoms consecutive atoms at a time: lane s tests candidate s of each atom's skin row with the exact
+// predicate; the index and atom loads of all of them are issued before the first test (the kernel is bound by the latency
+// of the scattered 32-byte atom reads), hits are compacted into nbr_idx by ballot.
+constexpr int kFilterAtoms = 4;
+
+__global__ void __launch_bounds__(kNbrWarps * 32)
+k_filter(Grid g, Basis bs, int n, int mmax, int smax, const AtomS* __restrict__ atoms, const int* __restrict__ skin_cnt,
+         const int* __restrict__ skin_idx, int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx,
+         unsigned char* __restrict__ nmask, unsigned long long* __restrict__ hitmask, int* __restrict__ flags) {
+    const int lane = threadIdx.x & 31;
+    const int k0 = (blockIdx.x * kNbrWarps + (threadIdx.x >> 5)) * kFilterAtoms;
+    if (k0 >= n) return;
+    int sc[kFilterAtoms], cnt[kFilterAtoms];
+    unsigned mask[kFilterAtoms];
+    unsigned long long hm[kFilterAtoms];
+    AtomS me[kFilterAtoms];
+    int scmax = 0;
+#pragma unroll
+    for (int a = 0; a < kFilterAtoms; a++) {
+        const int k = min(k0 + a, n - 1);
+        sc[a] = (k0 + a < n) ? skin_cnt[k] : 0;
+        me[a] = load_atom(atoms + k);
+        cnt[a] = 0; mask[a] = 0; hm[a] = 0;
+        scmax = max(scmax, sc[a]);
+    }
+    for (int base = 0; base < scmax; base += 32) {  // at most 2 passes (rows hold <= 64 candidates)
+        const int s = base + lane;
+        int j[kFilterAtoms];
+        AtomS o[kFilterAtoms];
+#pragma unroll
+        for (int a = 0; a < kFilterAtoms; a++) j[a] = (s < sc[a]) ? skin_idx[(size_t)(k0 + a) * smax + s] : 0;
+#pragma unroll
+        for (int a = 0; a < kFilterAtoms; a++) o[a] = load_atom(atoms + j[a]);
+#pragma unroll
+        for (int a = 0; a < kFilterAtoms; a++) {
+            double dx, dy, dz;
+            displacement(g, me[a], o[a], dx, dy, dz);
+            const bool hit = (s < sc[a]) && dist2_canonical(dx, dy, dz) < bs.rc2[me[a].type * bs.S + o[a].type];  // strict (R6)
+            const unsigned b = __ballot_sync(kFull, hit);
+            if (hit) {
+                const int slot = cnt[a] + __popc(b & ((1u << lane) - 1u));
+                if (slot < mmax) nbr_idx[(size_t)(k0 + a) * mmax + slot] = j[a];
+                mask[a] |= 1u << o[a].type;
+            }
+            cnt[a] += __popc(b);
+            hm[a] |= (unsigned long long)b << base;
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < kFilterAtoms; a++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mask[a] |= __shfl_xor_sync(kFull, mask[a], o);
+        if (lane == 0 && k0 + a < n) {
+            if (cnt[a] > mmax) { atomicOr(flags, kFlagNeighborOverflow); cnt[a] = mmax; }
+            nbr_cnt[k0 + a] = cnt[a];
+            nmask[k0 + a] = (unsigned char)mask[a];
+            hitmask[k0 + a] = hm[a];
+        }
+    }
+}
+
+// rev of the filtered list: the hit (k, s) sits in row j at the number of j's hits before k's candidate slot there
+__global__ void __launch_bounds__(kNbrWarps * 32)
+k_rev_from_skin(int n, int mmax, int smax, const int* __restrict__ skin_cnt, const int* __restrict__ skin_idx,
+                const unsigned char* __restrict__ skin_rev, const unsigned long long* __restrict__ hitmask,
+                unsigned char* __restrict__ rev) {
+    const int lane = threadIdx.x & 31;
+    const int k0 = (blockIdx.x * kNbrWarps + (threadIdx.x >> 5)) * kFilterAtoms;
+    if (k0 >= n) return;
+    int sc[kFilterAtoms];
+    unsigned long long hm[kFilterAtoms];
+    int scmax = 0;
+#pragma unroll
+    for (int a = 0; a < kFilterAtoms; a++) {
+        const bool in = k0 + a < n;
+        sc[a] = in ? skin_cnt[k0 + a] : 0;
+        hm[a] = in ? hitmask[k0 + a] : 0ull;
+        scmax = max(scmax, sc[a]);
+    }
+    for (int base = 0; base < scmax; base += 32) {
+        const int s = base + lane;
+        bool on[kFilterAtoms];
+        int t[kFilterAtoms];
+        unsigned long long hj[kFilterAtoms];
+#pragma unroll
+        for (int a = 0; a < kFilterAtoms; a++) {
+            on[a] = s < sc[a] && ((hm[a] >> s) & 1ull);
+            const size_t q = (size_t)(k0 + a) * smax + s;
+            const int j = on[a] ? skin_idx[q] : 0;
+            t[a] = on[a] ? skin_rev[q] : 0;  // candidate slot of k in row j
+            hj[a] = hitmask[j];
+        }
+#pragma unroll
+        for (int a = 0; a < kFilterAtoms; a++) {
+            if (on[a]) {
+                const int slot = __popcll(hm[a] & ((1ull << s) - 1ull));
+                if (slot < mmax)
+                    rev[(size_t)(k0 + a) * mmax + slot] = (unsigned char)__popcll(hj[a] & ((1ull << t[a]) - 1ull));
+            }
+        }
     }
 }
 
@@ -449,28 +605,54 @@ k_group_assign(int n, int S, int sparse, int n_groups, const AtomS* __restrict__
 
 // ------------------------------------------------------------------ host-side driver of a1
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
-                     const int* types, int mmax, int sparse, int n_groups) {
+                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid) {
     if (n == 0) return;
     const int tb = 256;
+    const bool use_skin = skin > 0.0;
+    const int* gate = nullptr;
+    int* nbr_cnt = ws.nbr_cnt;
+    int* nbr_idx = ws.nbr_idx;
+    unsigned char* rev = ws.rev;
+    Basis bsb = bs;  // cutoffs of the list that is BUILT (r_cut + skin in skin mode)
+    int bmax = mmax;  // its row stride
+    if (use_skin) {
+        bmax = kSkinStride;
+        gate = ws.skin_gate;
+        nbr_cnt = ws.skin_cnt; nbr_idx = ws.skin_idx; rev = ws.skin_rev;
+        for (int i = 0; i < bs.S * bs.S; i++) bsb.rc2[i] = (bs.rc[i] + skin) * (bs.rc[i] + skin);
+        L.memset(ws.skin_gate, list_valid ? 0 : 1, sizeof(int));  // bytes of 0x01: non-zero = rebuild; [1] counts rebuilds
+        if (list_valid)  // threshold a hair under (skin/2)^2: the triangle inequality then holds with rounding to spare
+            L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order,
+                     (const AtomS*)ws.ref, 0.2499 * skin * skin, ws.atoms, ws.skin_gate, ws.flags);
+    }
     L.memset(ws.cell_cnt, 0, sizeof(int) * (size_t)g.n_cells);
     L.launch(k_cell_assign, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, ws.cell_of, ws.rank_in_cell, ws.cell_cnt,
-             ws.flags);
-    exclusive_scan(L, g.n_cells, ws.cell_cnt, ws.cell_start, ws.scan_tmp);
+             ws.flags, gate);
+    exclusive_scan(L, g.n_cells, ws.cell_cnt, ws.cell_start, ws.scan_tmp, gate);
     L.launch(k_scatter, dim3((n + tb - 1) / tb), dim3(tb), 0, n, (const int*)ws.cell_of, (const int*)ws.rank_in_cell,
-             (const int*)ws.cell_start, ws.order);
-    L.launch(k_sort_cells, dim3((g.n_cells + tb - 1) / tb), dim3(tb), 0, g.n_cells, (const int*)ws.cell_start, ws.order);
-    L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order, ws.atoms);
+             (const int*)ws.cell_start, ws.order, gate);
+    L.launch(k_sort_cells, dim3((g.n_cells + tb - 1) / tb), dim3(tb), 0, g.n_cells, (const int*)ws.cell_start, ws.order,
+             gate);
+    L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order, ws.atoms, gate);
     const int nwb = (n + kNbrWarps - 1) / kNbrWarps;
-    if (mmax <= 64) {
-        const size_t stage = sizeof(int) * kNbrThreads * (size_t)(mmax | 1);
-        L.launch(k_neighbors_tpa, dim3((n + kNbrThreads - 1) / kNbrThreads), dim3(kNbrThreads), stage, g, bs, n,
-                 (const AtomS*)ws.atoms, (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+    if (bmax <= 64) {
+        const size_t stage = sizeof(int) * kNbrThreads * (size_t)(bmax | 1);
+        L.launch(k_neighbors_tpa, dim3((n + kNbrThreads - 1) / kNbrThreads), dim3(kNbrThreads), stage, g, bsb, n,
+                 (const AtomS*)ws.atoms, (const int*)ws.cell_start, bmax, nbr_cnt, nbr_idx, ws.nmask, ws.flags, gate);
     } else {
-        L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bs, n, (const AtomS*)ws.atoms,
-                 (const int*)ws.cell_start, mmax, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.flags);
+        L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bsb, n, (const AtomS*)ws.atoms,
+                 (const int*)ws.cell_start, bmax, nbr_cnt, nbr_idx, ws.nmask, ws.flags, gate);
     }
-    L.launch(k_reverse_index, dim3(nwb), dim3(kNbrWarps * 32), 0, n, mmax, (const int*)ws.nbr_cnt,
-             (const int*)ws.nbr_idx, ws.rev);
+    L.launch(k_reverse_index, dim3(nwb), dim3(kNbrWarps * 32), 0, n, bmax, (const int*)nbr_cnt, (const int*)nbr_idx, rev,
+             gate);
+    if (use_skin) {
+        L.launch(k_copy_ref, dim3((n + tb - 1) / tb), dim3(tb), 0, n, (const AtomS*)ws.atoms, ws.ref, gate, ws.skin_gate + 1);
+        const int nfb = (n + kNbrWarps * kFilterAtoms - 1) / (kNbrWarps * kFilterAtoms);
+        L.launch(k_filter, dim3(nfb), dim3(kNbrWarps * 32), 0, g, bs, n, mmax, bmax, (const AtomS*)ws.atoms,
+                 (const int*)ws.skin_cnt, (const int*)ws.skin_idx, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.hitmask, ws.flags);
+        L.launch(k_rev_from_skin, dim3(nfb), dim3(kNbrWarps * 32), 0, n, mmax, bmax, (const int*)ws.skin_cnt,
+                 (const int*)ws.skin_idx, (const unsigned char*)ws.skin_rev, (const unsigned long long*)ws.hitmask, ws.rev);
+    }
     const int ngb = (n + kGroupBlock - 1) / kGroupBlock;
     L.launch(k_group_hist, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
              (const unsigned char*)ws.nmask, ws.group_hist);

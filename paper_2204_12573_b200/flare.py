@@ -21,7 +21,7 @@ ERRORS = {
     -4: "FLARE_ERR_WORKSPACE_TOO_SMALL", -5: "FLARE_ERR_NEIGHBOR_OVERFLOW", -6: "FLARE_ERR_CUDA",
     -7: "FLARE_ERR_NONFINITE", -8: "FLARE_ERR_UNSUPPORTED", -9: "FLARE_ERR_NOT_BOUND",
 }
-OPT_MAX_NEIGHBORS, OPT_CHUNK_ATOMS, OPT_TIMING, OPT_SPECIES_SPARSE = 1, 2, 3, 4
+OPT_MAX_NEIGHBORS, OPT_CHUNK_ATOMS, OPT_TIMING, OPT_SPECIES_SPARSE, OPT_SKIN, OPT_SKIN_REBUILDS = 1, 2, 3, 4, 5, 6
 PHASES = ("neighbor", "descriptor", "qform", "backprop", "gather", "integrate")
 
 # every symbol include/flare_b200.h declares (checked by the CPU test-suite)
@@ -117,7 +117,7 @@ class Flare:
 
     def __init__(self, mass, n_max: int, l_max: int, r_cut, beta, sigma=None, device: int = 0,
                  max_neighbors: int | None = None, chunk_atoms: int | None = None, timing: bool = False,
-                 species_sparse: bool | None = None):
+                 species_sparse: bool | None = None, skin: float | None = None):
         import torch  # device memory + stream only
 
         self._torch = torch
@@ -152,6 +152,8 @@ class Flare:
             self.set_option(OPT_TIMING, 1)
         if species_sparse is not None:
             self.set_option(OPT_SPECIES_SPARSE, 1 if species_sparse else 0)
+        if skin is not None:
+            self.set_option(OPT_SKIN, int(round(1e3 * skin)))  # Angstrom -> 1e-3 Angstrom
 
     # ------------------------------------------------------------------ plumbing
     def _check(self, rc: int):

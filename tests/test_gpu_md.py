@@ -121,3 +121,39 @@ def test_supplied_forces_skip_the_initial_evaluation(torch, flare):
     n1 = ctx3.kernel_launches()
     ctx3.step(1.0, 2)
     assert ctx3.kernel_launches() - n1 > per_eval  # that one evaluated the initial forces as well
+
+
+def test_skin_list_reuse_is_exact(oracle, torch, flare):
+    """The candidate list with a skin (R12) is reused across steps and rebuilt on the device when an atom has moved
+    skin/2: trajectories agree with the rebuild-every-step path to rounding, the neighbour sets at the end are the
+    oracle's bit for bit, and the run really did both reuse and rebuild the list."""
+    s = w.config2()
+    out = {}
+    for skin in (0.0, 0.4):
+        ctx = start(torch, flare, s, skin=skin)
+        ctx.step(0.5, 60, want_variance=True)
+        st = ctx.get_state_host(variances=True)
+        out[skin] = (ctx, st)
+    (c0, a), (c1, b) = out[0.0], out[0.4]
+    assert c0.get_option(flare.OPT_SKIN) == 0 and c1.get_option(flare.OPT_SKIN) == 400
+    rebuilds = c1.get_option(flare.OPT_SKIN_REBUILDS)
+    assert 1 < rebuilds < 61, rebuilds          # 61 evaluations: some rebuilt, most reused
+    assert c0.get_option(flare.OPT_SKIN_REBUILDS) == 0
+    assert np.abs(a["pos"] - b["pos"]).max() < 1e-9
+    assert np.abs(a["F"] - b["F"]).max() < 1e-7
+    cnt_g, idx_g = c1.neighbors()
+    cnt_o, idx_o = oracle.neighbors(b["pos"], s.types, s.box, s.pbc, s.r_cut, 0, cap=idx_g.shape[1])
+    assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+    E, F, V = oracle.compute(b["pos"], s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, nbr_method=0)
+    assert np.all(np.abs(b["E"] - E) <= 1e-12 + 1e-10 * np.abs(E))
+    assert np.all(np.abs(b["F"] - F) <= 1e-12 + 1e-10 * np.abs(F))
+    assert np.all(np.abs(b["V"] - V) <= 1e-15 + 1e-10 * np.abs(V))
+    # a jump of one atom far beyond the skin (new positions through set_state) forces a rebuild and stays exact
+    pos2 = b["pos"].copy()
+    pos2[900] += np.array([3.0, -2.0, 1.5])
+    c1.set_state(pos2, b["vel"], s.types, s.box, s.pbc)
+    c1.step(0.5, 0, want_variance=False)
+    assert c1.get_option(flare.OPT_SKIN_REBUILDS) == rebuilds + 1
+    cnt_g, idx_g = c1.neighbors()
+    cnt_o, idx_o = oracle.neighbors(pos2, s.types, s.box, s.pbc, s.r_cut, 0, cap=idx_g.shape[1])
+    assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)

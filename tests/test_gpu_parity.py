@@ -289,7 +289,10 @@ def test_many_neighbours_more_than_a_warp(oracle, torch, flare):
     s = _mk(pos, np.zeros(len(keep)), np.diag([30.0, 30, 30]).reshape(9), [1, 1, 1], 1, n_max=3, l_max=2, seed=22)
     cnt, _ = oracle.neighbors(s.pos, s.types, s.box, s.pbc, s.r_cut, 0, cap=255)
     assert cnt.max() > 40
-    assert_parity(oracle, torch, flare, s, nbr_method=0, max_neighbors=int(cnt.max()) + 1)
+    # a blob this dense has more than 64 candidates within r_cut + skin: the candidate list is switched off
+    assert_parity(oracle, torch, flare, s, nbr_method=0, max_neighbors=int(cnt.max()) + 1, skin=0.0)
+    with pytest.raises(flare.FlareError):
+        gpu_compute(torch, flare, s, max_neighbors=int(cnt.max()) + 1, skin=0.4)
 
 
 def test_host_entry_point_matches_device_entry_point(torch, flare):
