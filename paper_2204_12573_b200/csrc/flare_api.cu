@@ -249,7 +249,7 @@ struct Carver {
 int auto_chunk(const flare_ctx* c, int64_t n) {
     if (c->chunk_opt > 0) return (int)std::min<int64_t>(std::max<int64_t>(c->chunk_opt, 1), std::max<int64_t>(n, 1));
     const double per_row = 8.0 * (c->bs.NvL2 + 2.0 * c->ld + 1 + 2.0 * c->max_ntn);
-    int64_t rows = (int64_t)(4.0 * 1024 * 1024 * 1024 / per_row);
+    int64_t rows = (int64_t)(16.0 * 1024 * 1024 * 1024 / per_row);  // 16 GiB of chunk intermediates (of 180 GB)
     rows = std::max<int64_t>(rows, 16384);
     return (int)std::max<int64_t>(1, std::min<int64_t>(rows, n));
 }
