@@ -320,6 +320,75 @@ def test_tile_16k_atoms_sampled(oracle, torch, flare):
     assert np.abs(f.sum(0)).max() < 1e-9
 
 
+def test_config3_full_size_sampled(oracle, torch, flare):
+    """BASELINE.json config 3 at full size (1 082 016 atoms, P = 544, variance on) in the launch configuration
+    bench.py times (default options: species-sparse groups, skin list, automatic chunk), after MD steps so that the
+    reused candidate list is what produced the neighbour sets: sampled atoms of every group against the oracle,
+    one by one; neighbour sets of the sampled atoms bit-exact; properties that hold at any size for the rest."""
+    s = w.config3()
+    ctx = flare.from_system(s).bind(s.n_atoms)
+    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)
+    ctx.step(0.5, 3, want_variance=True)
+    st = ctx.get_state_host(variances=True)
+    assert ctx.get_option(flare.OPT_SKIN_REBUILDS) < 4  # 4 evaluations, at least one on a reused list
+    groups = ctx.groups()
+    assert sum(r for r, _ in groups) == s.n_atoms and {p for r, p in groups if r} == {144, 544}
+    pos, types = st["pos"], s.types
+    n_pt = int(np.sum(types == 0))
+    rng = np.random.default_rng(33)
+    cnt_g, idx_g = ctx.neighbors()
+    # sample: Pt atoms at random, H atoms at random, plus atoms whose neighbourhood holds both species (P_g = 544)
+    sel = np.concatenate([rng.choice(n_pt, 20, replace=False), n_pt + rng.choice(s.n_atoms - n_pt, 10, replace=False)])
+    cand = rng.choice(s.n_atoms, 40000, replace=False)
+    both = [i for i in cand if cnt_g[i] and len(set(types[idx_g[i, :cnt_g[i]]].tolist())) == 2][:10]
+    assert len(both) == 10
+    sel = np.concatenate([sel, np.array(both)]).astype(np.int64)
+    E, F, V = oracle.compute_selected(pos, types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, sel)
+    assert_close(st["E"][sel], E, ATOL_E, "E")
+    assert_close(st["F"][sel], F, ATOL_F, "F")
+    assert_close(st["V"][sel], V, 1e-15, "V")
+    # neighbour sets of the sampled atoms: brute force against all N atoms with the canonical arithmetic (R6)
+    L = np.asarray(s.box, float).reshape(3, 3).diagonal()
+    xw = oracle.wrap(pos, s.box, s.pbc)
+    for i in sel[:12]:
+        d = xw - xw[i]
+        for a in range(3):
+            if s.pbc[a]:
+                d[:, a] = np.where(d[:, a] > 0.5 * L[a], d[:, a] - L[a], np.where(d[:, a] < -0.5 * L[a], d[:, a] + L[a], d[:, a]))
+        d2 = (d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2]
+        rc = np.asarray(s.r_cut, float).reshape(2, 2)[types[i], types]
+        nb = np.nonzero((d2 < rc * rc) & (np.arange(s.n_atoms) != i))[0]
+        assert np.array_equal(nb, idx_g[i, :cnt_g[i]])
+    # any-size properties: symmetric list, zero net force, finite outputs
+    assert cnt_g.sum() % 2 == 0
+    assert np.abs(st["F"].sum(0)).max() < 1e-7
+    assert np.isfinite(st["E"]).all() and np.isfinite(st["F"]).all() and np.isfinite(st["V"]).all()
+
+
+def test_config4_full_size_sampled(oracle, torch, flare):
+    """BASELINE.json config 4 (9 994 400 atoms): one evaluation with the default options, sampled atoms against the
+    oracle one by one, plus the any-size properties; also reports the workspace bytes per atom."""
+    s = w.config4()
+    ctx = flare.from_system(s).bind(s.n_atoms)
+    pos = torch.as_tensor(s.pos, dtype=torch.float64, device="cuda")
+    types = torch.as_tensor(s.types, dtype=torch.int32, device="cuda")
+    e, f, v = ctx.compute(pos, types, s.box, s.pbc, variances=True)
+    torch.cuda.synchronize()
+    assert ctx.get_option(2) < s.n_atoms  # several atom chunks (a8)
+    per_atom = ctx.workspace_bytes(s.n_atoms) / s.n_atoms
+    assert per_atom < 4096, per_atom      # 1.9 KB persistent + 16 GiB of chunk intermediates
+    n_pt = int(np.sum(s.types == 0))
+    rng = np.random.default_rng(44)
+    sel = np.concatenate([rng.choice(n_pt, 12, replace=False), n_pt + rng.choice(s.n_atoms - n_pt, 6, replace=False)])
+    E, F, V = oracle.compute_selected(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, sel)
+    sel_t = torch.as_tensor(sel, device="cuda")
+    assert_close(e[sel_t].cpu().numpy(), E, ATOL_E, "E")
+    assert_close(f[sel_t].cpu().numpy(), F, ATOL_F, "F")
+    assert_close(v[sel_t].cpu().numpy(), V, 1e-15, "V")
+    assert float(f.sum(0).abs().max()) < 1e-6
+    assert bool(torch.isfinite(e).all()) and bool(torch.isfinite(f).all()) and bool(torch.isfinite(v).all())
+
+
 def test_isolated_atoms_in_sparse_mode(oracle, torch, flare):
     """Atoms without neighbours form an empty (species, mask=0) group: E = V = 0, no forces, no table reads."""
     rng = np.random.default_rng(51)
