@@ -334,7 +334,7 @@ def run_ours(args):
     P = s.P
     sparse = bool(ctx.get_option(flare.OPT_SPECIES_SPARSE))
     groups = [g for g in ctx.groups() if g[0] > 0]
-    flops_per_step = ctx.qform_flops(want_var)  # sum over atoms of 2 P_g^2 per form (P_g = P without sparsity)
+    flops_per_step = ctx.qform_flops(want_var)  # sum over atoms of 2 P_g^2 per form
     qf_bytes_per_step = float(sum(r * 8.0 * p * (2 if want_var else 1) + r * 8.0 * p for r, p in groups))
     qf_ms, qf_launches = phases["qform"]
     qf_ms_per_step = qf_ms / args.steps
@@ -359,6 +359,10 @@ def run_ours(args):
                        "(MEASURED_PEAKS.json has no FP64 entry; its sustained bf16 x nominal 45/2250 gives "
                        f"{derived:.1f} TFLOP/s)" if derived else "FP64 DMMA issue peak measured live",
         "flops_per_launch_set": flops_per_step, "ms_per_step": qf_ms_per_step,
+        # the variance tiles skip the blocks of the symmetric Sigma below the diagonal: flops the kernel really needs
+        "flops_needed_with_symmetry": ctx.qform_flops(want_var, symmetric=True),
+        "frac_of_needed_flops": (ctx.qform_flops(want_var, symmetric=True) / (qf_ms_per_step * 1e-3) * 1e-12 / peak
+                                 if qf_ms_per_step > 0 and peak > 0 else None),
         "launches_per_step": qf_launches / args.steps,
         "share_of_step": qf_ms_per_step / ms_per_step,
     }

@@ -128,7 +128,8 @@ double eff_skin(const flare_ctx* c) { return c->mmax <= kSkinStride ? c->skin : 
 
 // choose the tile width (in n8 blocks) that wastes the fewest padded columns; ties -> wider tile
 void choose_tiles(int K, int& nb, int& ntn) {
-    static const int cand[] = {18, 17, 16, 15, 14, 13, 12, 11, 10, 9, 8, 6, 4, 2};
+    // even widths only: a tile then starts on a 16-column super-block (the variance tiles' triangular schedule)
+    static const int cand[] = {18, 16, 14, 12, 10, 8, 6, 4, 2};
     const int n8 = K / 8;
     long best = -1;
     nb = 2; ntn = (n8 + 1) / 2;

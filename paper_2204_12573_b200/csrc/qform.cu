@@ -109,10 +109,21 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
             cp_async16(bs + r * kQfLds + 2 * c, M + (size_t)r * a.K + k0 + 2 * c, 16);
         }
     };
+    // Variance tiles use the symmetry of Sigma: V = sum_{n,k} Sigma[n,k] d_n d_k only needs the 16 x 16 super-blocks with
+    // n-block >= k-block, the strictly upper ones counted twice, so a variance tile stops at the K slab that holds its
+    // last column and skips the column blocks left of the current slab (about half the DMMAs).  Energy tiles need all of
+    // W = beta d (it feeds dE/dB), so they stay dense.
+    auto tile_nk = [&](int tile) {
+        const int rem = tile % tiles_per_m;
+        const int mat = rem / a.ntn;
+        const int nt = rem - mat * a.ntn;
+        return mat == 0 ? nk : min(nk, (nt * BN + BN - 1) / kQfBK + 1);
+    };
     auto prologue = [&](int tile) {
+        const int nkt = tile_nk(tile);
 #pragma unroll
         for (int s = 0; s < STAGES - 1; s++) {
-            if (s < nk) load_stage(tile, s, s);
+            if (s < nkt) load_stage(tile, s, s);
             cp_async_commit();
         }
     };
@@ -132,22 +143,53 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
 #pragma unroll
             for (int nb = 0; nb < NB; nb++) { acc[h][nb][0] = 0.0; acc[h][nb][1] = 0.0; }
 
-        for (int kt = 0; kt < nk; kt++) {
+        const int nkt = tile_nk(tile);
+        const int nB0 = (nt * BN) / kQfBK;  // first 16-wide super-block of the tile's columns
+        for (int kt = 0; kt < nkt; kt++) {
             cp_async_wait<STAGES - 2>();
             __syncthreads();
-            if (kt + STAGES - 1 < nk) load_stage(tile, kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
+            if (kt + STAGES - 1 < nkt) load_stage(tile, kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
             cp_async_commit();
             const double* as = As + (kt % STAGES) * BM * kQfLds + (warp * 16 + g8) * kQfLds + t4;
             const double* bs = Bs + (kt % STAGES) * BN * kQfLds + g8 * kQfLds + t4;
+            if (mat == 0) {
 #pragma unroll
-            for (int ks = 0; ks < kQfBK / 4; ks++) {
-                const double a0 = as[4 * ks];
-                const double a1 = as[8 * kQfLds + 4 * ks];
+                for (int ks = 0; ks < kQfBK / 4; ks++) {
+                    const double a0 = as[4 * ks];
+                    const double a1 = as[8 * kQfLds + 4 * ks];
 #pragma unroll
-                for (int nb = 0; nb < NB; nb++) {
-                    const double b = bs[nb * 8 * kQfLds + 4 * ks];
-                    dmma884(acc[0][nb][0], acc[0][nb][1], a0, b);
-                    dmma884(acc[1][nb][0], acc[1][nb][1], a1, b);
+                    for (int nb = 0; nb < NB; nb++) {
+                        const double b = bs[nb * 8 * kQfLds + 4 * ks];
+                        dmma884(acc[0][nb][0], acc[0][nb][1], a0, b);
+                        dmma884(acc[1][nb][0], acc[1][nb][1], a1, b);
+                    }
+                }
+            } else {
+                // super-block of column block nb relative to the slab: rel = rel0 + nb / 2; < 0: not needed, 0: diagonal
+                // (counted once), > 0: strictly upper (counted twice).  Skipping is decided per GROUP of 6 column blocks
+                // (one warp-uniform branch, the 12 DMMAs inside stay one straight-line block); blocks of an active group
+                // that are not needed run with a zero operand.
+                const int rel0 = nB0 - kt;
+#pragma unroll
+                for (int ks = 0; ks < kQfBK / 4; ks++) {
+                    const double a0 = as[4 * ks];
+                    const double a1 = as[8 * kQfLds + 4 * ks];
+                    const double a0d = 2.0 * a0, a1d = 2.0 * a1;
+#pragma unroll
+                    for (int gb = 0; gb < NB; gb += 6) {
+                        constexpr int kLastOfGroup = 5;
+                        if (rel0 + min(gb + kLastOfGroup, NB - 1) / 2 >= 0) {  // the group's last super-block is needed
+#pragma unroll
+                            for (int nb = gb; nb < gb + 6 && nb < NB; nb++) {
+                                const int rel = rel0 + nb / 2;
+                                const double x0 = rel < 0 ? 0.0 : (rel > 0 ? a0d : a0);
+                                const double x1 = rel < 0 ? 0.0 : (rel > 0 ? a1d : a1);
+                                const double b = bs[nb * 8 * kQfLds + 4 * ks];
+                                dmma884(acc[0][nb][0], acc[0][nb][1], x0, b);
+                                dmma884(acc[1][nb][0], acc[1][nb][1], x1, b);
+                            }
+                        }
+                    }
                 }
             }
         }

@@ -348,9 +348,19 @@ class Flare:
         self._check(self._lib.flare_get_groups(self._ctx, C.cast(C.byref(n), C.c_void_p), _hp(rows), _hp(comps)))
         return [(int(rows[g]), int(comps[g])) for g in range(n.value)]
 
-    def qform_flops(self, variance: bool) -> float:
-        """Algorithmic flops of steps a4 (+ a5): sum over atoms of 2 P_g^2 per form."""
-        return float(sum(r * 2.0 * p * p for r, p in self.groups()) * (2 if variance else 1))
+    def qform_flops(self, variance: bool, symmetric: bool = False) -> float:
+        """Flops of steps a4 (+ a5) per evaluation.  Default: SURVEY.md 8(d)'s algorithmic count, 2 P_g^2 per atom and
+        per form.  symmetric=True: what the kernel needs since the variance tiles use the symmetry of Sigma -- all of
+        W = beta d (it feeds the forces) but only the 16 x 16 blocks of Sigma on and above the diagonal (512 flops each)."""
+        tot = 0.0
+        for r, p in self.groups():
+            tot += r * 2.0 * p * p
+            if variance and symmetric:
+                nsb = (p + 15) // 16
+                tot += r * 512.0 * (nsb * (nsb + 1) // 2)
+            elif variance:
+                tot += r * 2.0 * p * p
+        return float(tot)
 
     def timings(self):
         ms = np.zeros(len(PHASES))
