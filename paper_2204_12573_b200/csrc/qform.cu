@@ -269,7 +269,12 @@ static void launch_qform(Launcher& L, const QfArgs& a, int sm_count, long long m
     }
     // persistent grid: MINB CTAs per SM, but never more CTAs than the chunk could give tiles
     const long long max_tiles = ((max_m_rows + C::BM - 1) / C::BM) * a.ntn * a.n_mat;
-    const long long cap = (long long)sm_count * C::MINB;
+    static int occ = 0;  // resident CTAs per SM of this instantiation (narrow tiles need few registers: more than MINB fit)
+    if (occ == 0) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_qform<NB, WARPS>, C::THREADS, smem) != cudaSuccess || occ < 1)
+            occ = C::MINB;
+    }
+    const long long cap = (long long)sm_count * occ;
     const int grid = (int)(max_tiles < cap ? max_tiles : cap);
     L.launch(k_qform<NB, WARPS>, dim3(grid), dim3(C::THREADS), smem, a);
 }
