@@ -288,12 +288,16 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
                             int mmax, const GroupRun& gr, int ld, int chunk_cap, int max_ntn, bool want_variance) {
     using SM = BpSmem<LMAX, NMAXP>;
     const int Nc8 = (gr.Nc + 7) & ~7;
-    // atoms per warp: as many as keep a warp's shared memory near 14 KB (4 CTAs per SM), at least 1, at most 8
+    // atoms per warp (1..8): the most that do not cost resident CTAs.  With one atom per warp ctas1 CTAs of kBpWarps warps
+    // fit in an SM's shared memory (at most 4 matter: 128 registers per thread); more atoms per warp pack more pairs
+    // into each 32-lane pass, so take the largest count that still lets min(ctas1, 4) CTAs fit.
     int ta = kBpMaxTA;
     if (gr.nsp > 0) {
-        const int budget = 1792 - 2 * (Nc8 * SM::AS + 2 * gr.K);
-        ta = budget / (gr.nsp * SM::GB);
-        ta = ta < 1 ? 1 : (ta > kBpMaxTA ? kBpMaxTA : ta);
+        const size_t sm_bytes = 227 * 1024;
+        auto cta_bytes = [&](int t) { return sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(t, gr.nsp, Nc8, gr.K); };
+        int target = (int)(sm_bytes / cta_bytes(1));
+        target = target > 4 ? 4 : (target < 1 ? 1 : target);
+        while (ta > 1 && cta_bytes(ta) * target > sm_bytes) ta--;
     }
     // warps per CTA: as many of kBpWarps as fit the 227 KB of shared memory a CTA can have (large (n_max, l_max))
     const size_t per_warp = sizeof(double) * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
