@@ -349,9 +349,9 @@ def run_ours(args):
     roofline = {
         "bound": "tensor", "kernel": "k_qform (FP64 DMMA grouped GEMM, beta + Sigma forms)",
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak > 0 else None,
-        # dram__bytes_read+write of k_qform per row, from the ncu --set full capture in profiles/r01c_qform_full.md
-        # (2 251 B per K=144 row, 5 556 B per K=544 row, variance on), scaled to one step's rows
-        "traffic": (float(sum(r * {144: 2251.0, 544: 5556.0}[p] for r, p in groups))
+        # dram__bytes_read+write of k_qform per row, from the ncu --set full capture in profiles/r01f_c3.md
+        # (3 290 B per K=144 row, 5 860 B per K=544 row, variance on), scaled to one step's rows
+        "traffic": (float(sum(r * {144: 3290.0, 544: 5860.0}[p] for r, p in groups))
                     if want_var and all(p in (144, 544) for _, p in groups) else None),
         "algorithmic_bytes": qf_bytes_per_step,
         "groups_rows_x_components": groups,
