@@ -304,6 +304,7 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.red = cv.take<double>((size_t)kRedBlocksMax * 9);
     w.scal = cv.take<double>(16);
     w.ascal = cv.take<unsigned long long>(18);
+    w.qf_counter = cv.take<int>(kMaxGroups);
     if (ws) *ws = w;
     if (chunk_out) *chunk_out = chunk;
     if (cells_out) *cells_out = (int)std::min<size_t>(cells, 0x7fffffff);

@@ -82,6 +82,7 @@ struct Workspace {
     double* red = nullptr;                 // [kRedBlocksMax][9] per-block partial sums
     double* scal = nullptr;                // [16]: [0..8] virial, [12..15] thermostat xi, eta, scale, K2
     unsigned long long* ascal = nullptr;   // [18] analysis outputs (max bits, count, coordination histogram)
+    int* qf_counter = nullptr;             // [kMaxGroups] tile queues of the quadratic-form launches
 };
 constexpr int kRedBlocksMax = 1184;
 

@@ -36,6 +36,7 @@ struct QfArgs {
     int n_mat;            // 1 (energy only) or 2 (+variance)
     int chunk_cap;
     int max_ntn;
+    int* counter;         // tile queue of this launch (zeroed before it)
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src, int src_bytes) {
@@ -128,7 +129,12 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
         }
     };
 
-    int tile = blockIdx.x;
+    // Tiles are handed out through a counter: variance tiles are cheaper than energy tiles, so a static assignment
+    // (tile += gridDim.x keeps a CTA on one kind when the grid is even) left half of the CTAs idle at the end.
+    __shared__ int s_tile;
+    if (tid == 0) s_tile = atomicAdd(a.counter, 1);
+    __syncthreads();
+    int tile = s_tile;
     if (tile < total) prologue(tile);
     while (tile < total) {
         const int mt = tile / tiles_per_m;
@@ -196,7 +202,9 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
         // all warps are done with the stages: refill the pipeline for the next tile, so that its first
         // slabs arrive while this tile's epilogue runs
         __syncthreads();
-        const int next = tile + gridDim.x;
+        if (tid == 0) s_tile = atomicAdd(a.counter, 1);
+        __syncthreads();
+        const int next = s_tile;
         if (next < total) prologue(next);
 
         // ---- fused epilogue: W store (energy tiles) + partial row-dot with B of the same columns
@@ -285,6 +293,7 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
     int max_ntn = 0;
     for (int g = 0; g < n_groups; g++) max_ntn = groups[g].ntn > max_ntn ? groups[g].ntn : max_ntn;
     const int variant = qf_variant();
+    L.memset(ws.qf_counter, 0, sizeof(int) * kMaxGroups);
     for (int g = 0; g < n_groups; g++) {
         const GroupDesc& gd = groups[g];
         if (gd.K == 0 || gd.beta == nullptr) continue;
@@ -294,6 +303,7 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
         a.g = g; a.row0 = row0; a.nrows = nrows; a.ld = ld; a.K = gd.K; a.ntn = gd.ntn;
         a.n_mat = (want_variance && gd.sigma) ? 2 : 1;
         a.chunk_cap = chunk_cap; a.max_ntn = max_ntn;
+        a.counter = ws.qf_counter + g;
         switch (gd.nb) {
 #define FLARE_CASE(NBV)                                                   \
     case NBV:                                                             \
