@@ -249,7 +249,8 @@ def run_ours(args):
     n = s.n_atoms
     ctx = flare.from_system(s, device=local, variance=want_var, timing=True,
                             chunk_atoms=args.chunk if args.chunk else None,
-                            species_sparse=False if args.dense else None, skin=args.skin)
+                            species_sparse=False if args.dense else None, skin=args.skin,
+                            max_neighbors=args.max_neighbors)
     ctx.bind(n)
     dt_fs = float(s.meta.get("dt_fs", 0.5))
     pos = torch.as_tensor(s.pos, dtype=torch.float64, device=dev)
@@ -373,6 +374,7 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "atoms": n, "P": P, "variance": want_var, "dt_fs": dt_fs,
                    "species_sparse": sparse, "skin_angstrom": 1e-3 * ctx.get_option(flare.OPT_SKIN),
+                   "max_neighbors": ctx.get_option(flare.OPT_MAX_NEIGHBORS),
                    "chunk_atoms": ctx.get_option(flare.OPT_CHUNK_ATOMS),
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": "working set (>10 GB of descriptors per step) is far larger than the 126 MB L2; no flush needed"},
@@ -402,6 +404,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-variance", action="store_true")
     ap.add_argument("--dense", action="store_true", help="switch the species-sparse evaluation (P:L155) off")
+    ap.add_argument("--max-neighbors", type=int, default=None, help="row stride of the neighbour table (library default 48)")
     ap.add_argument("--skin", type=float, default=None, help="skin of the candidate neighbour list in Angstrom (0 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomposed", action="store_true",
