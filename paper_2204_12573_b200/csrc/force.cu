@@ -1,12 +1,13 @@
 // force.cu -- steps a6 + a7: back-propagation of dE/dB through A to per-pair forces, and the
 // atomics-free force gather ("reordering the summation" so that grad d_i is never formed).
 //
-// k_backprop, one warp per atom k (row of the current chunk):
-//   E_k   = sum of the energy tiles' partial row-dots (fixed order)           (Eq. 1)
-//   V_k   = same for the variance tiles                                        (Eq. 2)
-//   c_p   = dE_k/dB_p = (2/||B||)(W_p - E_k B^_p),  W = beta B^               (R10, R11)
-//   G[nu1,lm] = dE_k/dA[nu1,lm] = sum_{nu2} c_{p(nu1,nu2,l)} (1+delta) A[nu2,lm]
-//   f_kj  = dE_k/dr_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj)   for every neighbour j
+// k_backprop, one launch per (chunk, group), a warp per block of up to 8 rows (atoms) k:
+//   E_k   = sum of the energy tiles' partial row-dots (fixed order) / ||B||^2     (Eq. 1; rows hold unnormalised B)
+//   V_k   = same for the variance tiles                                            (Eq. 2)
+//   c_p   = dE_k/dB_p = (2/||B||^2)(W_p - E_k B_p),  W = beta B                   (R10, R11)
+//   G[nu1,lm] = dE_k/dA[nu1,lm] = sum_{nu2} c_{p(nu1,nu2,l)} (1+delta) A[nu2,lm]   (FP64 tensor pipe)
+//   f_kj  = dE_k/dr_kj = sum_{n,lm} G[s_j n, lm] grad(g~_n Y_lm)(r_kj)   for every neighbour j, one pair per lane over
+//           the concatenated neighbour lists of the warp's atoms
 // f_kj is stored once per ordered pair.  k_gather then forms, with the reverse-pair index,
 //   F_k = sum_j ( f_kj - f_jk )
 // reading each pair force exactly twice and writing each atom's force exactly once.

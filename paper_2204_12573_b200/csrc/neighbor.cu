@@ -2,6 +2,10 @@
 // radius"; R5-R7).  Produces, in cell-sorted atom order, a FULL (symmetric) neighbour
 // table nbr_idx[N][mmax] + nbr_cnt[N], the reverse-pair index rev[N][mmax] used by the atomics-free
 // force gather, the neighbour-species bitmask, and the grouping of atoms into quadratic-form rows.
+// With a skin (the default, R22) the build chain makes a CANDIDATE list with cutoffs r_cut + skin and
+// only runs when a device-side gate says an atom has moved skin/2 since the last build; every evaluation
+// refreshes the sorted positions and filters the candidates with the exact predicate (k_refresh, k_filter,
+// k_rev_from_skin), so the neighbour sets themselves are always exact.
 #include "kernels.cuh"
 
 namespace flare {

@@ -2,16 +2,19 @@
 // (Eq. 1-2), batched over the atoms of a group as a dense FP64 contraction
 //     W[rows x K] = B^[rows x K] . M[K x K],   M = beta^(s) or Sigma^(s) (symmetric, K = padded P),
 // on the FP64 tensor pipe (mma.sync.m8n8k4.f64 -> DMMA.8x8x4; tcgen05 has no f64 kind).
-// The paper does this one atom per block as a mat-vec; here the descriptor rows of up to
-// 128 atoms share every tile of the matrix.
+// The paper does this one atom per block as a mat-vec; here the descriptor rows of 64 atoms
+// share every tile of the matrix.
 //
-// Tiling: CTA tile 128 rows x (8*NB) columns, 8 warps stacked along M (16 rows each), every warp
-// spans the full tile width, so the row-dots of the epilogue never cross warps.  K is streamed in
-// slabs of 16 through a 4-stage cp.async pipeline; shared-memory rows are padded to 20 doubles so
-// that the 8-byte fragment loads of a half-warp hit 16 distinct banks pairs.
-// Epilogue (fused): energy tiles store W (needed for dE/dB) and the partial row-dot
-// sum_n W[r][n] B^[r][n]; variance tiles store only the partial row-dot.  Partials of the ntn tiles
+// Tiling: CTA tile 64 rows x (8*NB) columns, 4 warps stacked along M (16 rows each), every warp spans
+// the full tile width, so the row-dots of the epilogue never cross warps; two CTAs per SM, tiles taken
+// from a device counter.  K is streamed in slabs of 16 through a 3-stage cp.async pipeline (the next
+// tile's first slabs are requested before the epilogue); shared-memory rows are padded to 20 doubles so
+// that the 8-byte fragment loads of a half-warp hit 16 distinct bank pairs.  Variance tiles use the
+// symmetry of Sigma (upper 16 x 16 super-blocks only).
+// Epilogue (fused): energy tiles store W = beta B (needed for dE/dB) and the partial row-dot
+// sum_n W[r][n] B[r][n]; variance tiles store only the partial row-dot.  Partials of the ntn tiles
 // of a row are summed in fixed order by the back-propagation kernel (deterministic, atomics-free).
+// The rows hold the UNNORMALISED B; the 1/||B||^2 factor is applied by the back-propagation kernel.
 #include <cstdlib>
 
 #include "kernels.cuh"
