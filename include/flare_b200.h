@@ -62,10 +62,11 @@ enum {
                                     ("dividing atoms into batches"); 0 = automatic (default) */
     FLARE_OPT_TIMING = 3,        /* 1: bracket every kernel phase with CUDA events (flare_get_timings) */
     FLARE_OPT_SKIN_MILLI_ANGSTROM = 5, /* skin of the candidate neighbour list in 1e-3 Angstrom (default 400; 0 = off).
-                                    With a skin the cell-sorted order and a list of all pairs within r_cut + skin are
-                                    kept across evaluations; every evaluation filters it with the exact predicate (R6,
-                                    R12: the neighbour sets stay exact) and rebuilds it, on the device, as soon as an
-                                    atom has moved skin/2 since the last build.  Candidate rows hold at most 64 entries
+                                    With a skin the cell-sorted order and a list of all pairs within max r_cut + skin
+                                    are kept across evaluations; every evaluation filters it with the exact predicate
+                                    (R6, R12: the neighbour sets stay exact) and rebuilds it, on the device, as soon as
+                                    two atoms of species a, b could have closed max r_cut + skin - r_cut[a][b] between
+                                    them since the last build.  Candidate rows hold at most 64 entries
                                     (more: FLARE_ERR_NEIGHBOR_OVERFLOW; lower the skin).  Costs 360 B/atom. */
     FLARE_OPT_SKIN_REBUILDS = 6,  /* read-only (flare_get_option, synchronises): candidate-list rebuilds since flare_bind */
     FLARE_OPT_SPECIES_SPARSE = 4 /* 1 (default when S * 2^S <= 64): atoms are grouped by the set of neighbour species

@@ -291,7 +291,7 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
         w.skin_rev = cv.take<unsigned char>(N * kSkinStride);
         w.ref = cv.take<AtomS>(N);
         w.hitmask = cv.take<unsigned long long>(N);
-        w.skin_gate = cv.take<int>(4);
+        w.skin_gate = cv.take<int>(4 + kMaxSpecies);  // gate, rebuild count, -, -, per-species max displacement
     }
     w.pairf = cv.take<double>(N * c->mmax * 3);
     w.e_s = cv.take<double>(N);

@@ -394,31 +394,59 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
 // above runs again), and filters the candidates with the exact canonical predicate.  The reverse-pair index of the
 // filtered list follows from the candidate list's own reverse index and the per-atom hit masks, without any search.
 
-// sorted positions <- current positions (in the order of the last build); raise the gate if anyone moved too far
-__global__ void k_refresh(Grid g, int n, const double* __restrict__ pos, const int* __restrict__ types,
-                          const int* __restrict__ order, const AtomS* __restrict__ ref, double half_skin2,
-                          AtomS* __restrict__ atoms, int* __restrict__ gate, int* __restrict__ flags) {
+// sorted positions <- current positions (in the order of the last build); per-species maximum displacement since the
+// build (as the bits of a float rounded up: non-negative floats order like their bit patterns) -> dmax[S]
+__global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, const int* __restrict__ types,
+                          const int* __restrict__ order, const AtomS* __restrict__ ref, AtomS* __restrict__ atoms,
+                          int* __restrict__ gate, int* __restrict__ dmax, int* __restrict__ flags) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n) return;
-    const int i = order[k];
-    double p[3] = {pos[3 * (size_t)i], pos[3 * (size_t)i + 1], pos[3 * (size_t)i + 2]};
-    bool bad = false;
+    int my_type = -1;
+    int bits = 0;
+    if (k < n) {
+        const int i = order[k];
+        double p[3] = {pos[3 * (size_t)i], pos[3 * (size_t)i + 1], pos[3 * (size_t)i + 2]};
+        bool bad = false;
 #pragma unroll
-    for (int d = 0; d < 3; d++) {
-        if (!isfinite(p[d])) { bad = true; p[d] = 0.0; }
-        if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
+        for (int d = 0; d < 3; d++) {
+            if (!isfinite(p[d])) { bad = true; p[d] = 0.0; }
+            if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
+        }
+        AtomS a;
+        a.x = p[0]; a.y = p[1]; a.z = p[2];
+        a.type = types[i];
+        a.orig = i;
+        atoms[k] = a;
+        const AtomS r = load_atom(ref + k);
+        double dx, dy, dz;
+        displacement(g, r, a, dx, dy, dz);
+        const double d2 = dx * dx + dy * dy + dz * dz;
+        if (bad) atomicOr(flags, kFlagNonFinite);
+        if (bad || !(d2 < 1e30) || r.type != a.type) *gate = 1;  // benign race: every writer stores 1
+        my_type = a.type;
+        bits = __float_as_int(__double2float_ru(sqrt(d2)));
     }
-    AtomS a;
-    a.x = p[0]; a.y = p[1]; a.z = p[2];
-    a.type = types[i];
-    a.orig = i;
-    atoms[k] = a;
-    const AtomS r = load_atom(ref + k);
-    double dx, dy, dz;
-    displacement(g, r, a, dx, dy, dz);
-    const bool moved = bad || !(dx * dx + dy * dy + dz * dz < half_skin2) || r.type != a.type;
-    if (bad) atomicOr(flags, kFlagNonFinite);
-    if (moved) *gate = 1;  // benign race: every writer stores 1
+    // one atomic per (warp, species present in the warp)
+    for (int s = 0; s < S; s++) {
+        int m = (my_type == s) ? bits : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(kFull, m, o));
+        if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(dmax + s, m);
+    }
+}
+
+// A pair (a, b) of the candidate list (cutoff rc_max + skin for every pair) stays complete while
+// d_a + d_b < (rc_max + skin) - r_cut[a][b]: the pairs with the largest cutoff have `skin` to spend, pairs with a
+// shorter cutoff (every pair with an H in the H2/Pt workloads) much more, so the fast light atoms do not force
+// rebuilds.  The threshold is taken a hair low so that the triangle inequality holds with rounding to spare.
+__global__ void k_gate_decide(Basis bs, double reach, const int* __restrict__ dmax, int* __restrict__ gate) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int need = 0;
+    for (int a = 0; a < bs.S; a++)
+        for (int b = a; b < bs.S; b++) {
+            const double da = __int_as_float(dmax[a]), db = __int_as_float(dmax[b]);
+            if (!(da + db < 0.9998 * (reach - bs.rc[a * bs.S + b]))) need = 1;
+        }
+    if (need) *gate = 1;
 }
 
 __global__ void k_copy_ref(int n, const AtomS* __restrict__ atoms, AtomS* __restrict__ ref, const int* __restrict__ gate,
@@ -625,11 +653,17 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
         bmax = kSkinStride;
         gate = ws.skin_gate;
         nbr_cnt = ws.skin_cnt; nbr_idx = ws.skin_idx; rev = ws.skin_rev;
-        for (int i = 0; i < bs.S * bs.S; i++) bsb.rc2[i] = (bs.rc[i] + skin) * (bs.rc[i] + skin);
+        double rcmax = 0.0;
+        for (int i = 0; i < bs.S * bs.S; i++) rcmax = bs.rc[i] > rcmax ? bs.rc[i] : rcmax;
+        const double reach = rcmax + skin;  // one candidate cutoff for every species pair
+        for (int i = 0; i < bs.S * bs.S; i++) bsb.rc2[i] = reach * reach;
         L.memset(ws.skin_gate, list_valid ? 0 : 1, sizeof(int));  // bytes of 0x01: non-zero = rebuild; [1] counts rebuilds
-        if (list_valid)  // threshold a hair under (skin/2)^2: the triangle inequality then holds with rounding to spare
-            L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order,
-                     (const AtomS*)ws.ref, 0.2499 * skin * skin, ws.atoms, ws.skin_gate, ws.flags);
+        if (list_valid) {
+            L.memset(ws.skin_gate + 4, 0, sizeof(int) * kMaxSpecies);  // per-species maximum displacement
+            L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, bs.S, n, pos, types, (const int*)ws.order,
+                     (const AtomS*)ws.ref, ws.atoms, ws.skin_gate, ws.skin_gate + 4, ws.flags);
+            L.launch(k_gate_decide, dim3(1), dim3(32), 0, bs, reach, (const int*)(ws.skin_gate + 4), ws.skin_gate);
+        }
     }
     L.memset(ws.cell_cnt, 0, sizeof(int) * (size_t)g.n_cells);
     L.launch(k_cell_assign, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, ws.cell_of, ws.rank_in_cell, ws.cell_cnt,
