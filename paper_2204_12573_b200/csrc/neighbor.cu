@@ -354,44 +354,45 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
                 unsigned char* __restrict__ rev, const int* __restrict__ gate) {
     if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     const int lane = threadIdx.x & 31;
-    const int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5);
-    if (k >= n) return;
-    const int cnt = nbr_cnt[k];
-    for (int base = 0; base < cnt; base += 32) {
-        const int s = base + lane;
-        const int nact = min(32, cnt - base);
-        int j = 0, cj = 0;
-        if (s < cnt) { j = nbr_idx[(size_t)k * mmax + s]; cj = nbr_cnt[j]; }
-        int mine = 0;
-        for (int t0 = 0; t0 < nact; t0 += 4) {
-            int jj[4], cc[4], v[4];
+    // grid-stride over atoms: a fixed, small grid, so that the gated (skipped) launch costs next to nothing
+    for (int k = blockIdx.x * kNbrWarps + (threadIdx.x >> 5); k < n; k += gridDim.x * kNbrWarps) {
+        const int cnt = nbr_cnt[k];
+        for (int base = 0; base < cnt; base += 32) {
+            const int s = base + lane;
+            const int nact = min(32, cnt - base);
+            int j = 0, cj = 0;
+            if (s < cnt) { j = nbr_idx[(size_t)k * mmax + s]; cj = nbr_cnt[j]; }
+            int mine = 0;
+            for (int t0 = 0; t0 < nact; t0 += 4) {
+                int jj[4], cc[4], v[4];
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
-                jj[u] = __shfl_sync(kFull, j, (t0 + u) & 31);
-                cc[u] = __shfl_sync(kFull, cj, (t0 + u) & 31);  // 0 beyond nact: nothing is read
-                v[u] = (lane < cc[u]) ? nbr_idx[(size_t)jj[u] * mmax + lane] : -1;
-            }
-#pragma unroll
-            for (int u = 0; u < 4; u++) {
-                unsigned m = __ballot_sync(kFull, v[u] == k);
-                int found = m ? __ffs(m) - 1 : 0;
-                for (int b = 32; !m && b < cc[u]; b += 32) {  // rows longer than a warp
-                    const int t = b + lane;
-                    m = __ballot_sync(kFull, (t < cc[u]) && (nbr_idx[(size_t)jj[u] * mmax + t] == k));
-                    if (m) found = b + __ffs(m) - 1;
+                for (int u = 0; u < 4; u++) {
+                    jj[u] = __shfl_sync(kFull, j, (t0 + u) & 31);
+                    cc[u] = __shfl_sync(kFull, cj, (t0 + u) & 31);  // 0 beyond nact: nothing is read
+                    v[u] = (lane < cc[u]) ? nbr_idx[(size_t)jj[u] * mmax + lane] : -1;
                 }
-                if (lane == t0 + u) mine = found;
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    unsigned m = __ballot_sync(kFull, v[u] == k);
+                    int found = m ? __ffs(m) - 1 : 0;
+                    for (int b = 32; !m && b < cc[u]; b += 32) {  // rows longer than a warp
+                        const int t = b + lane;
+                        m = __ballot_sync(kFull, (t < cc[u]) && (nbr_idx[(size_t)jj[u] * mmax + t] == k));
+                        if (m) found = b + __ffs(m) - 1;
+                    }
+                    if (lane == t0 + u) mine = found;
+                }
             }
+            if (s < cnt) rev[(size_t)k * mmax + s] = (unsigned char)mine;
         }
-        if (s < cnt) rev[(size_t)k * mmax + s] = (unsigned char)mine;
     }
 }
 
 // ------------------------------------------------------------------ skin list (R12: "a skin list filtered by the exact
 // predicate is allowed, sets must still be exact").  Between rebuilds the cell-sorted order and a candidate list built
-// with cutoffs r_cut + skin are kept; every evaluation refreshes the sorted positions, checks that no atom has moved
-// further than skin/2 from where it was when the list was built (else the gate is raised and the whole build chain
-// above runs again), and filters the candidates with the exact canonical predicate.  The reverse-pair index of the
+// with the cutoff max r_cut + skin are kept; every evaluation refreshes the sorted positions, checks the per-species
+// displacements since the build against the budget of every species pair (else the gate is raised and the whole build
+// chain above runs again), and filters the candidates with the exact canonical predicate.  The reverse-pair index of the
 // filtered list follows from the candidate list's own reverse index and the per-atom hit masks, without any search.
 
 // sorted positions <- current positions (in the order of the last build); per-species maximum displacement since the
@@ -683,7 +684,7 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
         L.launch(k_neighbors, dim3(nwb), dim3(kNbrWarps * 32), 0, g, bsb, n, (const AtomS*)ws.atoms,
                  (const int*)ws.cell_start, bmax, nbr_cnt, nbr_idx, ws.nmask, ws.flags, gate);
     }
-    L.launch(k_reverse_index, dim3(nwb), dim3(kNbrWarps * 32), 0, n, bmax, (const int*)nbr_cnt, (const int*)nbr_idx, rev,
+    L.launch(k_reverse_index, dim3(nwb < 148 * 32 ? nwb : 148 * 32), dim3(kNbrWarps * 32), 0, n, bmax, (const int*)nbr_cnt, (const int*)nbr_idx, rev,
              gate);
     if (use_skin) {
         L.launch(k_copy_ref, dim3((n + tb - 1) / tb), dim3(tb), 0, n, (const AtomS*)ws.atoms, ws.ref, gate, ws.skin_gate + 1);
