@@ -52,7 +52,8 @@ class CudaEngine(Engine):
         if self._ws is None:
             self.ctx.bind(self.capacity)  # allocates the workspace for the capacity
             self._ws = self.ctx._workspace
-        self.ctx.bind(n, workspace=self._ws)
+        if self.ctx.n_atoms != n:  # re-binding drops the candidate neighbour list: only when the size changed
+            self.ctx.bind(n, workspace=self._ws)
 
     def evaluate(self, pos, types, box, pbc, variances):
         self._bind(pos.shape[0])
