@@ -157,3 +157,65 @@ def test_skin_list_reuse_is_exact(oracle, torch, flare):
     cnt_g, idx_g = c1.neighbors()
     cnt_o, idx_o = oracle.neighbors(pos2, s.types, s.box, s.pbc, s.r_cut, 0, cap=idx_g.shape[1])
     assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+
+
+@pytest.mark.parametrize("case", ["open_z", "two_cells", "hot_gas"])
+def test_skin_list_edge_geometries(oracle, torch, flare, case):
+    """The reused candidate list in the geometries where its bookkeeping could go wrong: an open dimension with atoms
+    leaving the box, a periodic box only two cells wide (every cell is its own neighbour several times over), and a hot
+    two-species gas whose atoms cross cell and box boundaries every few steps.  After the run the neighbour sets must be
+    the oracle's bit for bit and E, F, V must agree at the final positions."""
+    rng = np.random.default_rng(77)
+    if case == "open_z":
+        s = w.tile_like_c3(10, 5, n_max=3, l_max=2)
+        s.pbc = np.array([1, 1, 0], np.int32)
+        s.vel = w.maxwell_velocities(rng, s.types, s.mass, 3000.0)
+        dt, steps = 1.0, 40
+    elif case == "two_cells":
+        pos, types, box, pbc = w.fcc_bulk(2, w.A_PT, 0.05, rng)  # L = 7.84 A: two cells of 3.9 A per dimension
+        s = w.System("two_cells", pos, types, box, pbc, np.array([w.MASS_PT]), np.array([[3.5]]), 3, 2)
+        P = w.num_descriptors(1, 3, 2)
+        s.beta, s.sigma = w.random_beta(rng, 1, P), w.random_sigma(rng, 1, P)
+        s.vel = w.maxwell_velocities(rng, s.types, s.mass, 20000.0)
+        dt, steps = 2.0, 60
+    else:
+        n = 300
+        L = 24.0
+        pos = rng.uniform(0, L, (n, 3))
+        keep = [0]
+        for i in range(1, n):
+            d = pos[keep] - pos[i]
+            d -= L * np.round(d / L)
+            if np.min(np.linalg.norm(d, axis=1)) > 1.3:
+                keep.append(i)
+        pos = pos[keep]
+        types = rng.integers(0, 2, len(keep)).astype(np.int32)
+        s = w.System("hot_gas", pos, types, np.diag([L, L, L]).reshape(9), np.ones(3, np.int32),
+                     np.array([w.MASS_PT, w.MASS_H]), w.R_CUT_2, 3, 2)
+        P = w.num_descriptors(2, 3, 2)
+        s.beta, s.sigma = w.random_beta(rng, 2, P), w.random_sigma(rng, 2, P)
+        s.vel = w.maxwell_velocities(rng, s.types, s.mass, 4000.0)
+        dt, steps = 1.0, 60
+    ctx = start(torch, flare, s)
+    assert ctx.get_option(flare.OPT_SKIN) == 400
+    ctx.step(dt, steps, want_variance=True)
+    st = ctx.get_state_host(variances=True)
+    rebuilds = ctx.get_option(flare.OPT_SKIN_REBUILDS)
+    assert 1 <= rebuilds <= steps + 1
+    cnt_g, idx_g = ctx.neighbors()
+    cnt_o, idx_o = oracle.neighbors(st["pos"], s.types, s.box, s.pbc, s.r_cut, 0, cap=idx_g.shape[1])
+    assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+    E, F, V = oracle.compute(st["pos"], s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, nbr_method=0)
+    assert np.all(np.abs(st["E"] - E) <= 1e-12 + 1e-10 * np.abs(E))
+    assert np.all(np.abs(st["F"] - F) <= 1e-12 + 1e-10 * np.abs(F))
+    assert np.all(np.abs(st["V"] - V) <= 1e-15 + 1e-10 * np.abs(V))
+    # the same run with the list rebuilt at every evaluation ends in the same place (to rounding)
+    ref = start(torch, flare, s, skin=0.0)
+    ref.step(dt, steps, want_variance=True)
+    rp = ref.get_state_host()["pos"]
+    d = st["pos"] - rp
+    L3 = np.asarray(s.box, float).reshape(3, 3).diagonal()
+    for a in range(3):
+        if s.pbc[a]:
+            d[:, a] -= L3[a] * np.round(d[:, a] / L3[a])
+    assert np.abs(d).max() < 1e-7
