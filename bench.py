@@ -277,7 +277,13 @@ def run_ours(args):
         sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
-    ctx.step(dt_fs, args.steps, want_var)
+    analysis = None
+    if args.analysis and want_var and s.mass.size > 1:
+        for _ in range(args.steps):
+            ctx.step(dt_fs, 1, want_var)
+            analysis = ctx.analyze(threshold=0.05, species_a=1, species_b=1, r_coord=1.0)  # synchronises
+    else:
+        ctx.step(dt_fs, args.steps, want_var)
     ev1.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else {}
@@ -377,6 +383,9 @@ def run_ours(args):
                    "max_neighbors": ctx.get_option(flare.OPT_MAX_NEIGHBORS),
                    "chunk_atoms": ctx.get_option(flare.OPT_CHUNK_ATOMS),
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "analysis_every_step": ({"max_uncertainty": analysis["max_unc"], "n_above_0.05": analysis["n_above"],
+                                            "h_coordination_hist": [int(x) for x in analysis["hist"][:4]]}
+                                           if analysis else None),
                    "l2": "working set (>10 GB of descriptors per step) is far larger than the 126 MB L2; no flush needed"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -407,6 +416,9 @@ def main():
     ap.add_argument("--max-neighbors", type=int, default=None, help="row stride of the neighbour table (library default 48)")
     ap.add_argument("--skin", type=float, default=None, help="skin of the candidate neighbour list in Angstrom (0 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--analysis", action="store_true",
+                    help="also run flare_analyze (maximum uncertainty + H-H coordination within 1 A) after every step "
+                         "inside the timed region, like the paper's production run (P:L247-249)")
     ap.add_argument("--decomposed", action="store_true",
                     help="N ranks share ONE system N times as long as C3 (slab decomposition + halo exchange, "
                          "paper_2204_12573_b200/halo.py) instead of running N replicas")
