@@ -87,30 +87,39 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
     const int g8 = lane >> 2, t4 = lane & 3;
     const int nk = a.K / kQfBK;
 
-    // tile -> (row block, matrix, column block); loads of one K slab of a tile into a stage
-    auto load_stage = [&](int tile, int kt, int stage) {
+    // tile -> (row block, matrix, column block), decoded ONCE per tile (the divisions are not paid per K slab)
+    struct TileCtx {
+        const double* Ag;  // first row of the tile in the B array
+        const double* M;   // first row (n) of the tile's columns in the symmetric matrix
+        int rows_here;
+    };
+    auto decode = [&](int tile) {
         const int mt = tile / tiles_per_m;
         const int rem = tile - mt * tiles_per_m;
         const int mat = rem / a.ntn;
         const int nt = rem - mat * a.ntn;
-        const double* M = (mat == 0 ? a.beta : a.sigma) + (size_t)nt * BN * a.K;  // rows n of the symmetric matrix
-        const int mrow0 = mt * BM;
-        const double* Ag = a.Bh + (size_t)(lrow0 + mrow0) * a.ld;
-        const int rows_here = min(BM, n_rows - mrow0);
+        TileCtx c;
+        c.M = (mat == 0 ? a.beta : a.sigma) + (size_t)nt * BN * a.K;
+        c.Ag = a.Bh + (size_t)(lrow0 + mt * BM) * a.ld;
+        c.rows_here = min(BM, n_rows - mt * BM);
+        return c;
+    };
+    // loads of one K slab of a tile into a stage
+    auto load_stage = [&](const TileCtx& c, int kt, int stage) {
         const int k0 = kt * kQfBK;
         double* as = As + stage * BM * kQfLds;
         double* bs = Bs + stage * BN * kQfLds;
 #pragma unroll
         for (int i = 0; i < (BM * 8) / THREADS; i++) {  // A slab: BM rows x 8 chunks of 16 B
             const int idx = tid + i * THREADS;
-            const int r = idx >> 3, c = idx & 7;
-            const bool ok = r < rows_here;
-            const double* src = Ag + (size_t)(ok ? r : 0) * a.ld + k0 + 2 * c;
-            cp_async16(as + r * kQfLds + 2 * c, src, ok ? 16 : 0);
+            const int r = idx >> 3, ch = idx & 7;
+            const bool ok = r < c.rows_here;
+            const double* src = c.Ag + (size_t)(ok ? r : 0) * a.ld + k0 + 2 * ch;
+            cp_async16(as + r * kQfLds + 2 * ch, src, ok ? 16 : 0);
         }
         for (int idx = tid; idx < BN * 8; idx += THREADS) {  // B slab: BN rows x 8 chunks
-            const int r = idx >> 3, c = idx & 7;
-            cp_async16(bs + r * kQfLds + 2 * c, M + (size_t)r * a.K + k0 + 2 * c, 16);
+            const int r = idx >> 3, ch = idx & 7;
+            cp_async16(bs + r * kQfLds + 2 * ch, c.M + (size_t)r * a.K + k0 + 2 * ch, 16);
         }
     };
     // Variance tiles use the symmetry of Sigma: V = sum_{n,k} Sigma[n,k] d_n d_k only needs the 16 x 16 super-blocks with
@@ -125,9 +134,10 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
     };
     auto prologue = [&](int tile) {
         const int nkt = tile_nk(tile);
+        const TileCtx c = decode(tile);
 #pragma unroll
         for (int s = 0; s < STAGES - 1; s++) {
-            if (s < nkt) load_stage(tile, s, s);
+            if (s < nkt) load_stage(c, s, s);
             cp_async_commit();
         }
     };
@@ -154,10 +164,11 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
 
         const int nkt = tile_nk(tile);
         const int nB0 = (nt * BN) / kQfBK;  // first 16-wide super-block of the tile's columns
+        const TileCtx ctx = decode(tile);
         for (int kt = 0; kt < nkt; kt++) {
             cp_async_wait<STAGES - 2>();
             __syncthreads();
-            if (kt + STAGES - 1 < nkt) load_stage(tile, kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
+            if (kt + STAGES - 1 < nkt) load_stage(ctx, kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
             cp_async_commit();
             const double* as = As + (kt % STAGES) * BM * kQfLds + (warp * 16 + g8) * kQfLds + t4;
             const double* bs = Bs + (kt % STAGES) * BN * kQfLds + g8 * kQfLds + t4;
