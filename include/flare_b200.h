@@ -50,7 +50,7 @@ enum {
     FLARE_ERR_WORKSPACE_TOO_SMALL = -4,
     FLARE_ERR_NEIGHBOR_OVERFLOW = -5,  /* an atom has more than FLARE_OPT_MAX_NEIGHBORS neighbours */
     FLARE_ERR_CUDA = -6,               /* CUDA runtime error; message in flare_last_error */
-    FLARE_ERR_NONFINITE = -7,          /* NaN/Inf met in positions */
+    FLARE_ERR_NONFINITE = -7,          /* NaN/Inf met in positions, or produced in an energy, force or variance */
     FLARE_ERR_UNSUPPORTED = -8,        /* (n_max, l_max) outside the compiled range */
     FLARE_ERR_NOT_BOUND = -9           /* call needs flare_bind / flare_set_state first */
 };
@@ -127,8 +127,9 @@ int flare_bind(flare_ctx* ctx, int64_t n_atoms, void* workspace, size_t bytes, v
  *   pbc   [3] host, non-zero = periodic
  *   e_out [N] device or NULL; f_out [N][3] device or NULL; var_out [N] device or NULL
  *         (NULL var_out skips the Sigma form entirely).
- * Asynchronous.  Device-detected failures (neighbour overflow, non-finite input) are reported
- * by flare_check(), which synchronises.
+ * Asynchronous.  Device-detected failures (neighbour overflow, species out of range, non-finite input or
+ * output) are reported by flare_check(), which synchronises; after such a failure the kept candidate list is
+ * dropped, so the next evaluation starts from scratch.
  */
 int flare_compute(flare_ctx* ctx, const double* pos, const int32_t* types, const double box[9],
                   const int pbc[3], double* e_out, double* f_out, double* var_out);
@@ -219,6 +220,13 @@ int flare_get_descriptors(flare_ctx* ctx, double* bhat, double* nrm);
 int flare_get_groups(flare_ctx* ctx, int32_t* n_groups, int64_t* rows, int32_t* comps);
 
 /*
+ * Test hook (synchronises; HOST output): row[i] = quadratic-form row of atom i (caller's order) in the last
+ * evaluation.  Rows are ordered by group; chunk c of step a8 holds rows [c * chunk, (c+1) * chunk) with
+ * chunk = flare_get_option(FLARE_OPT_CHUNK_ATOMS), so tests can pick atoms next to a chunk boundary.
+ */
+int flare_get_rows(flare_ctx* ctx, int32_t* row);
+
+/*
  * Accumulated CUDA-event time (ms) and launch count per phase since the last call
  * (needs FLARE_OPT_TIMING = 1); ms and launches are [FLARE_N_PHASES] host arrays.  Synchronises.
  */
@@ -226,10 +234,6 @@ int flare_get_timings(flare_ctx* ctx, double* ms, int64_t* launches);
 
 /* Number of kernels the library has launched on this context since creation. */
 int64_t flare_kernel_launches(const flare_ctx* ctx);
-
-/* FP64 tensor-pipe (DMMA) issue peak of the device in TFLOP/s, measured by a register-resident
-   mma.sync m8n8k4 f64 loop: the roofline denominator of the quadratic-form kernel.  Synchronous. */
-double flare_measure_fp64_dmma_peak(int cuda_device);
 
 const char* flare_last_error(const flare_ctx* ctx);
 

@@ -153,7 +153,8 @@ k_ke_partial(int n, const double* __restrict__ v, const int* __restrict__ types,
     __shared__ double sm[kRedThreads / 32];
     double t[1] = {0.0};
     for (int i = blockIdx.x * kRedThreads + threadIdx.x; i < n; i += gridDim.x * kRedThreads) {
-        const double m = mass[types[i]];
+        const int ty = types[i];
+        const double m = (unsigned)ty < (unsigned)kMaxSpecies ? mass[ty] : 0.0;
         const double vx = v[3 * (size_t)i], vy = v[3 * (size_t)i + 1], vz = v[3 * (size_t)i + 2];
         t[0] += m * (vx * vx + vy * vy + vz * vz) * inv_kappa;
     }

@@ -228,11 +228,7 @@ static void launch_descriptor(Launcher& L, const Grid& g, const Basis& bs, const
     using SM = DescSmem<LMAX, NMAXP>;
     const int Nc8 = (gr.Nc + 7) & ~7;
     const size_t smem = sizeof(double) * kDescWarps * (size_t)SM::warp_doubles(Nc8);
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(k_descriptor<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = smem;
-    }
+    L.ensure_smem(k_descriptor<LMAX, NMAXP>, smem);
     const int per_cta = kDescWarps * kDescTA;
     L.launch(k_descriptor<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(kDescWarps * 32), smem, g, bs, yn,
              gr, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,

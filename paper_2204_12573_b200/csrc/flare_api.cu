@@ -76,11 +76,20 @@ struct flare_ctx {
     int pbc[3]{};
     // bookkeeping
     int64_t launches = 0;
+    LaunchCache launch_cache;  // per-context (= per-device) kernel attributes and occupancies
     PhaseEvents phases[FLARE_N_PHASES];
     std::string err;
 };
 
 namespace {
+
+Launcher make_launcher(flare_ctx* c) {
+    Launcher L;
+    L.stream = c->stream;
+    L.launch_count = &c->launches;
+    L.cache = &c->launch_cache;
+    return L;
+}
 
 int fail(flare_ctx* c, int code, const std::string& msg) {
     if (c) c->err = msg;
@@ -127,7 +136,8 @@ int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // the skin list needs one 64-bit hit mask per atom: rows longer than 64 switch it off
 double eff_skin(const flare_ctx* c) { return c->mmax <= kSkinStride ? c->skin : 0.0; }
 
-// choose the tile width (in n8 blocks) that wastes the fewest padded columns; ties -> wider tile
+// choose the tile width (in n8 blocks): the WIDEST one that pads the matrix by at most 5 % (wide tiles reuse the
+// B rows more and leave fewer partial row-dots: K = 544 -> 5 tiles of 112, not 17 of 32); if none, the least padding
 void choose_tiles(int K, int& nb, int& ntn) {
     // even widths only: a tile then starts on a 16-column super-block (the variance tiles' triangular schedule)
     static const int cand[] = {18, 16, 14, 12, 10, 8, 6, 4, 2};
@@ -135,8 +145,9 @@ void choose_tiles(int K, int& nb, int& ntn) {
     long best = -1;
     nb = 2; ntn = (n8 + 1) / 2;
     for (int c : cand) {
-        int t = (n8 + c - 1) / c;
-        long width = (long)t * c;
+        const int t = (n8 + c - 1) / c;
+        const long width = (long)t * c;
+        if (width * 100 <= (long)n8 * 105) { nb = c; ntn = t; return; }
         if (best < 0 || width < best) { best = width; nb = c; ntn = t; }
     }
 }
@@ -357,9 +368,7 @@ int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
 // ---------------------------------------------------------------- one evaluation (steps a1-a8)
 int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, double* f_out, double* var_out) {
     const int n = (int)c->n;
-    Launcher L;
-    L.stream = c->stream;
-    L.launch_count = &c->launches;
+    Launcher L = make_launcher(c);
     const bool want_var = (var_out != nullptr) && c->has_sigma;
     if (var_out && !c->has_sigma) return fail(c, FLARE_ERR_INVALID_ARG, "variance requested but the model has no sigma");
     if (n == 0) return FLARE_OK;
@@ -579,10 +588,20 @@ int flare_check(flare_ctx* c) {
     FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
     int flags[4] = {0, 0, 0, 0};
     FLARE_CUDA(c, cudaMemcpy(flags, c->ws.flags, sizeof(flags), cudaMemcpyDeviceToHost));
-    if (flags[0]) FLARE_CUDA(c, cudaMemset(c->ws.flags, 0, sizeof(flags)));
+    if (flags[0]) {
+        FLARE_CUDA(c, cudaMemset(c->ws.flags, 0, sizeof(flags)));
+        // whatever went wrong, the kept candidate list and pair forces may be truncated or built from bad input:
+        // the next evaluation rebuilds from scratch (and raises the error again if its cause persists)
+        c->list_valid = false;
+        c->pairf_valid = false;
+        c->forces_valid = c->var_valid = false;
+    }
+    if (flags[0] & kFlagBadType) return fail(c, FLARE_ERR_INVALID_ARG, "a species index is outside 0..S-1");
     if (flags[0] & kFlagNonFinite) return fail(c, FLARE_ERR_NONFINITE, "non-finite position");
     if (flags[0] & kFlagNeighborOverflow)
         return fail(c, FLARE_ERR_NEIGHBOR_OVERFLOW, "an atom has more neighbours than FLARE_OPT_MAX_NEIGHBORS (or more than 64 candidates within r_cut + skin: lower FLARE_OPT_SKIN_MILLI_ANGSTROM)");
+    if (flags[0] & kFlagNonFiniteResult)
+        return fail(c, FLARE_ERR_NONFINITE, "a non-finite energy, force or variance was produced (atoms too close, or a blown-up step)");
     return FLARE_OK;
 }
 
@@ -680,9 +699,7 @@ static int step_impl(flare_ctx* c, double dt_fs, int n_steps, int want_variance,
                                       cudaMemcpyHostToDevice, c->stream));
         c->accel_dt = dt_fs;
     }
-    Launcher L;
-    L.stream = c->stream;
-    L.launch_count = &c->launches;
+    Launcher L = make_launcher(c);
     const bool nvt = T_kelvin > 0.0;
     const double gkT = (3.0 * (double)n - 3.0) * 8.617333262e-5 * T_kelvin;  // g k_B T, g = 3N - 3 (R13, R19)
     const double Q = gkT * tau_fs * tau_fs;
@@ -748,9 +765,7 @@ int flare_get_virial(flare_ctx* c, double virial[9]) {
     FLARE_CUDA(c, cudaSetDevice(c->device));
     for (int q = 0; q < 9; q++) virial[q] = 0.0;
     if (c->n == 0) return FLARE_OK;
-    Launcher L;
-    L.stream = c->stream;
-    L.launch_count = &c->launches;
+    Launcher L = make_launcher(c);
     run_virial(L, c->grid, c->ws, (int)c->n, c->mmax, c->ws.scal);
     if (L.err != cudaSuccess) return cuda_fail(c, L.err, "virial launch");
     FLARE_CUDA(c, cudaMemcpyAsync(virial, c->ws.scal, sizeof(double) * 9, cudaMemcpyDeviceToHost, c->stream));
@@ -775,9 +790,7 @@ int flare_analyze(flare_ctx* c, double unc_threshold, int species_a, int species
     FLARE_CUDA(c, cudaSetDevice(c->device));
     unsigned long long h[18] = {0};
     if (c->n > 0 && (want_unc || want_coord)) {
-        Launcher L;
-        L.stream = c->stream;
-        L.launch_count = &c->launches;
+        Launcher L = make_launcher(c);
         run_analyze(L, c->grid, c->ws, (int)c->n, c->mmax, want_unc, unc_threshold, species_a, species_b, r_coord,
                     want_coord, coord, c->ws.ascal);
         if (L.err != cudaSuccess) return cuda_fail(c, L.err, "analysis launch");
@@ -865,9 +878,7 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
     FLARE_CUDA(c, cudaMemcpy(h_aor.data(), c->ws.atom_of_row, sizeof(int) * n, cudaMemcpyDeviceToHost));
     FLARE_CUDA(c, cudaMemcpy(h_gid.data(), c->ws.gid, n, cudaMemcpyDeviceToHost));
     const auto& comps = c->sets[c->sparse].comps;
-    Launcher L;
-    L.stream = c->stream;
-    L.launch_count = &c->launches;
+    Launcher L = make_launcher(c);
     std::vector<double> hb, hn;
     for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
         const int nrows = std::min(c->chunk_cap, n - row0);
@@ -912,6 +923,23 @@ int flare_get_groups(flare_ctx* c, int32_t* n_groups, int64_t* rows, int32_t* co
     return FLARE_OK;
 }
 
+int flare_get_rows(flare_ctx* c, int32_t* row) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->have_grid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    if (!row) return fail(c, FLARE_ERR_INVALID_ARG, "bad output array");
+    rc = flare_check(c);
+    if (rc) return rc;
+    const size_t n = (size_t)c->n;
+    if (n == 0) return FLARE_OK;
+    std::vector<AtomS> h_atoms(n);
+    std::vector<int> h_row(n);
+    FLARE_CUDA(c, cudaMemcpy(h_atoms.data(), c->ws.atoms, sizeof(AtomS) * n, cudaMemcpyDeviceToHost));
+    FLARE_CUDA(c, cudaMemcpy(h_row.data(), c->ws.row_of, sizeof(int) * n, cudaMemcpyDeviceToHost));
+    for (size_t k = 0; k < n; k++) row[h_atoms[k].orig] = h_row[k];
+    return FLARE_OK;
+}
+
 int flare_get_timings(flare_ctx* c, double* ms, int64_t* launches) {
     if (!c || !ms) return FLARE_ERR_INVALID_ARG;
     FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -931,8 +959,6 @@ int flare_get_timings(flare_ctx* c, double* ms, int64_t* launches) {
 }
 
 int64_t flare_kernel_launches(const flare_ctx* c) { return c ? c->launches : 0; }
-
-double flare_measure_fp64_dmma_peak(int cuda_device) { return measure_dmma_peak(cuda_device); }
 
 const char* flare_last_error(const flare_ctx* c) { return c ? c->err.c_str() : "null context"; }
 

@@ -309,11 +309,7 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
         if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.err_where = "back-propagation: descriptor too large for shared memory"; }
         return;
     }
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(k_backprop<LMAX, NMAXP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = smem;
-    }
+    L.ensure_smem(k_backprop<LMAX, NMAXP>, smem);
     const int per_cta = warps * ta;
     L.launch(k_backprop<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(warps * 32), smem, g, bs, yn, gr,
              ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
@@ -349,7 +345,7 @@ __global__ void __launch_bounds__(kGatherWarps * 32)
 k_gather(int n, int mmax, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
          const int* __restrict__ nbr_idx, const unsigned char* __restrict__ rev, const double* __restrict__ pairf,
          const double* __restrict__ e_s, const double* __restrict__ v_s, double* __restrict__ e_out,
-         double* __restrict__ f_out, double* __restrict__ var_out) {
+         double* __restrict__ f_out, double* __restrict__ var_out, int* __restrict__ flags) {
     const int lane = threadIdx.x & 31;
     const int k = blockIdx.x * kGatherWarps + (threadIdx.x >> 5);
     if (k >= n) return;
@@ -366,9 +362,12 @@ k_gather(int n, int mmax, const AtomS* __restrict__ atoms, const int* __restrict
     fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
     if (lane == 0) {
         const int i = atoms[k].orig;
+        const double e = e_s[k], v = var_out ? v_s[k] : 0.0;
         if (f_out) { f_out[3 * (size_t)i] = fx; f_out[3 * (size_t)i + 1] = fy; f_out[3 * (size_t)i + 2] = fz; }
-        if (e_out) e_out[i] = e_s[k];
-        if (var_out) var_out[i] = v_s[k];
+        if (e_out) e_out[i] = e;
+        if (var_out) var_out[i] = v;
+        // a blown-up step must not go unnoticed (flare_check -> FLARE_ERR_NONFINITE)
+        if (!(isfinite(fx) && isfinite(fy) && isfinite(fz) && isfinite(e) && isfinite(v))) atomicOr(flags, kFlagNonFiniteResult);
     }
 }
 
@@ -376,7 +375,7 @@ void run_gather(Launcher& L, const Workspace& ws, int n, int mmax, double* e_out
     if (n <= 0) return;
     L.launch(k_gather, dim3((n + kGatherWarps - 1) / kGatherWarps), dim3(kGatherWarps * 32), 0, n, mmax,
              (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, (const unsigned char*)ws.rev,
-             (const double*)ws.pairf, (const double*)ws.e_s, (const double*)ws.v_s, e_out, f_out, var_out);
+             (const double*)ws.pairf, (const double*)ws.e_s, (const double*)ws.v_s, e_out, f_out, var_out, ws.flags);
 }
 
 }  // namespace flare

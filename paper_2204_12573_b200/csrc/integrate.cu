@@ -11,7 +11,8 @@ __global__ void k_kick_drift(Grid g, int n, double* __restrict__ x, double* __re
                              const double* __restrict__ accel_half_dt, double dt) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const double a = accel_half_dt[types[i]];
+    const int t = types[i];
+    const double a = (unsigned)t < (unsigned)kMaxSpecies ? accel_half_dt[t] : 0.0;  // a bad type is flagged by the evaluation
 #pragma unroll
     for (int d = 0; d < 3; d++) {
         const size_t q = 3 * (size_t)i + d;
@@ -27,7 +28,8 @@ __global__ void k_kick(int n, double* __restrict__ v, const double* __restrict__
                        const double* __restrict__ accel_half_dt) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const double a = accel_half_dt[types[i]];
+    const int t = types[i];
+    const double a = (unsigned)t < (unsigned)kMaxSpecies ? accel_half_dt[t] : 0.0;  // a bad type is flagged by the evaluation
 #pragma unroll
     for (int d = 0; d < 3; d++) {
         const size_t q = 3 * (size_t)i + d;

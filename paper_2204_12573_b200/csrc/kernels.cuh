@@ -2,6 +2,7 @@
 // the workspace layout, the stream/launch-count/timing wrapper, and the per-stage entry points.
 #pragma once
 #include <utility>
+#include <vector>
 
 #include "basis.cuh"
 #include "common.cuh"
@@ -12,12 +13,51 @@ constexpr int kMaxGroups = 64;  // quadratic-form groups: (central species) or (
 constexpr int kNumPhases = 6;
 constexpr int kSkinStride = 64;  // row stride of the skin (candidate) list: one 64-bit hit mask per atom
 
+// Per-context launch state: the dynamic shared-memory limit a kernel has been configured for and its occupancy.
+// cudaFuncSetAttribute acts on the CURRENT device only, so this lives in the context (one context = one device),
+// not in function-local statics: a second context on another GPU of the same process configures its own copy.
+struct LaunchCache {
+    struct Entry { const void* fn; size_t smem; int occ; };
+    std::vector<Entry> entries;
+    Entry& find(const void* fn) {
+        for (Entry& e : entries) if (e.fn == fn) return e;
+        entries.push_back(Entry{fn, 0, 0});
+        return entries.back();
+    }
+};
+
 // Launch wrapper: all kernels go to one stream; counts launches; keeps the first CUDA error.
 struct Launcher {
     cudaStream_t stream = nullptr;
     int64_t* launch_count = nullptr;
+    LaunchCache* cache = nullptr;
     cudaError_t err = cudaSuccess;
     const char* err_where = nullptr;
+
+    // raise the kernel's dynamic shared-memory limit (needed above 48 KB) once per context and size
+    template <class... KArgs>
+    void ensure_smem(void (*kernel)(KArgs...), size_t bytes) {
+        if (bytes <= 48 * 1024 || err != cudaSuccess) return;
+        LaunchCache::Entry local{nullptr, 0, 0};
+        LaunchCache::Entry& e = cache ? cache->find(reinterpret_cast<const void*>(kernel)) : local;
+        if (bytes <= e.smem) return;
+        cudaError_t rc = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (rc != cudaSuccess) { err = rc; err_where = "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)"; return; }
+        e.smem = bytes;
+    }
+    // resident CTAs per SM of a kernel at this block size / shared memory (queried once per context)
+    template <class... KArgs>
+    int occupancy(void (*kernel)(KArgs...), int threads, size_t smem, int fallback) {
+        LaunchCache::Entry local{nullptr, 0, 0};
+        LaunchCache::Entry& e = cache ? cache->find(reinterpret_cast<const void*>(kernel)) : local;
+        if (e.occ == 0) {
+            int occ = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess || occ < 1)
+                occ = fallback;
+            e.occ = occ;
+        }
+        return e.occ;
+    }
 
     template <class... KArgs, class... Args>
     void launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
@@ -159,7 +199,5 @@ void run_analyze(Launcher& L, const Grid& g, const Workspace& ws, int n, int mma
                  unsigned long long* out18);
 void run_nh_half(Launcher& L, const Workspace& ws, int n, const double* mass_dev, double h, double gkT, double Q,
                  double* thermo);
-
-double measure_dmma_peak(int device);
 
 }  // namespace flare

@@ -148,8 +148,9 @@ __global__ void k_sort_cells(int n_cells, const int* __restrict__ cell_start, in
     }
 }
 
-__global__ void k_gather_atoms(Grid g, int n, const double* __restrict__ pos, const int* __restrict__ types,
-                               const int* __restrict__ order, AtomS* __restrict__ atoms, const int* __restrict__ gate) {
+__global__ void k_gather_atoms(Grid g, int S, int n, const double* __restrict__ pos, const int* __restrict__ types,
+                               const int* __restrict__ order, AtomS* __restrict__ atoms, int* __restrict__ flags,
+                               const int* __restrict__ gate) {
     if (gate != nullptr && *gate == 0) return;  // skin list still valid: nothing to rebuild
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
@@ -162,7 +163,9 @@ __global__ void k_gather_atoms(Grid g, int n, const double* __restrict__ pos, co
         if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
     }
     a.x = p[0]; a.y = p[1]; a.z = p[2];
-    a.type = types[i];
+    int t = types[i];
+    if ((unsigned)t >= (unsigned)S) { atomicOr(flags, kFlagBadType); t = 0; }  // keeps every table index in bounds
+    a.type = t;
     a.orig = i;
     atoms[k] = a;
 }
@@ -414,7 +417,9 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
         }
         AtomS a;
         a.x = p[0]; a.y = p[1]; a.z = p[2];
-        a.type = types[i];
+        int t = types[i];
+        if ((unsigned)t >= (unsigned)S) { atomicOr(flags, kFlagBadType); t = 0; }
+        a.type = t;
         a.orig = i;
         atoms[k] = a;
         const AtomS r = load_atom(ref + k);
@@ -674,7 +679,8 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
              (const int*)ws.cell_start, ws.order, gate);
     L.launch(k_sort_cells, dim3((g.n_cells + tb - 1) / tb), dim3(tb), 0, g.n_cells, (const int*)ws.cell_start, ws.order,
              gate);
-    L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, n, pos, types, (const int*)ws.order, ws.atoms, gate);
+    L.launch(k_gather_atoms, dim3((n + tb - 1) / tb), dim3(tb), 0, g, bs.S, n, pos, types, (const int*)ws.order, ws.atoms,
+             ws.flags, gate);
     const int nwb = (n + kNbrWarps - 1) / kNbrWarps;
     if (bmax <= 64) {
         const size_t stage = sizeof(int) * kNbrThreads * (size_t)(bmax | 1);

@@ -15,8 +15,6 @@
 // sum_n W[r][n] B[r][n]; variance tiles store only the partial row-dot.  Partials of the ntn tiles
 // of a row are summed in fixed order by the back-propagation kernel (deterministic, atomics-free).
 // The rows hold the UNNORMALISED B; the 1/||B||^2 factor is applied by the back-propagation kernel.
-#include <cstdlib>
-
 #include "kernels.cuh"
 
 namespace flare {
@@ -270,32 +268,16 @@ __global__ void __launch_bounds__(QfCfg<WARPS>::THREADS, QfCfg<WARPS>::MINB) k_q
     cp_async_wait<0>();
 }
 
-static int qf_variant() {  // development knob: FLARE_QF_WARPS=8 selects the 128-row, one-CTA-per-SM tiling
-    static int v = -1;
-    if (v < 0) {
-        const char* e = getenv("FLARE_QF_WARPS");
-        v = (e && atoi(e) == 8) ? 8 : 4;
-    }
-    return v;
-}
-
 template <int NB, int WARPS>
 static void launch_qform(Launcher& L, const QfArgs& a, int sm_count, long long max_m_rows) {
     using C = QfCfg<WARPS>;
     constexpr int BN = 8 * NB;
     const size_t smem = sizeof(double) * C::STAGES * (C::BM + BN) * kQfLds;
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_qform<NB, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = true;
-    }
+    L.ensure_smem(k_qform<NB, WARPS>, smem);
     // persistent grid: MINB CTAs per SM, but never more CTAs than the chunk could give tiles
     const long long max_tiles = ((max_m_rows + C::BM - 1) / C::BM) * a.ntn * a.n_mat;
-    static int occ = 0;  // resident CTAs per SM of this instantiation (narrow tiles need few registers: more than MINB fit)
-    if (occ == 0) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_qform<NB, WARPS>, C::THREADS, smem) != cudaSuccess || occ < 1)
-            occ = C::MINB;
-    }
+    // resident CTAs per SM of this instantiation (narrow tiles need few registers: more than MINB fit)
+    const int occ = L.occupancy(k_qform<NB, WARPS>, C::THREADS, smem, C::MINB);
     const long long cap = (long long)sm_count * occ;
     const int grid = (int)(max_tiles < cap ? max_tiles : cap);
     L.launch(k_qform<NB, WARPS>, dim3(grid), dim3(C::THREADS), smem, a);
@@ -306,7 +288,6 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
     if (nrows <= 0) return;
     int max_ntn = 0;
     for (int g = 0; g < n_groups; g++) max_ntn = groups[g].ntn > max_ntn ? groups[g].ntn : max_ntn;
-    const int variant = qf_variant();
     L.memset(ws.qf_counter, 0, sizeof(int) * kMaxGroups);
     for (int g = 0; g < n_groups; g++) {
         const GroupDesc& gd = groups[g];
@@ -321,60 +302,15 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
         switch (gd.nb) {
 #define FLARE_CASE(NBV)                                                   \
     case NBV:                                                             \
-        if (variant == 8) launch_qform<NBV, 8>(L, a, sm_count, nrows);    \
-        else launch_qform<NBV, 4>(L, a, sm_count, nrows);                 \
+        launch_qform<NBV, 4>(L, a, sm_count, nrows);                      \
         break;
-            FLARE_CASE(2) FLARE_CASE(4) FLARE_CASE(6) FLARE_CASE(8) FLARE_CASE(9) FLARE_CASE(10) FLARE_CASE(11)
-            FLARE_CASE(12) FLARE_CASE(13) FLARE_CASE(14) FLARE_CASE(15) FLARE_CASE(16) FLARE_CASE(17) FLARE_CASE(18)
+            // even widths only (choose_tiles): a tile starts on a 16-column super-block
+            FLARE_CASE(2) FLARE_CASE(4) FLARE_CASE(6) FLARE_CASE(8) FLARE_CASE(10)
+            FLARE_CASE(12) FLARE_CASE(14) FLARE_CASE(16) FLARE_CASE(18)
 #undef FLARE_CASE
             default: if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.err_where = "qform tile width"; } break;
         }
     }
-}
-
-// ------------------------------------------------------------------ FP64 DMMA issue peak (roofline denominator)
-__global__ void k_dmma_peak(double* out, int iters, double a, double b) {
-    double c[8][2];
-#pragma unroll
-    for (int i = 0; i < 8; i++) { c[i][0] = threadIdx.x; c[i][1] = i; }
-    for (int it = 0; it < iters; it++) {
-#pragma unroll
-        for (int i = 0; i < 8; i++) dmma884(c[i][0], c[i][1], a, b);
-    }
-    double s = 0;
-#pragma unroll
-    for (int i = 0; i < 8; i++) s += c[i][0] + c[i][1];
-    if (s == 123.456) out[0] = s;
-}
-
-double measure_dmma_peak(int device) {
-    if (cudaSetDevice(device) != cudaSuccess) return -1.0;
-    cudaDeviceProp p;
-    if (cudaGetDeviceProperties(&p, device) != cudaSuccess) return -1.0;
-    double* out = nullptr;
-    if (cudaMalloc(&out, 8) != cudaSuccess) return -1.0;
-    const int blocks = p.multiProcessorCount * 2, threads = 256, iters = 1 << 14;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
-    k_dmma_peak<<<blocks, threads>>>(out, iters, 1.0000001, 1e-9);
-    cudaDeviceSynchronize();
-    float best = 1e30f;
-    for (int r = 0; r < 5; r++) {
-        cudaEventRecord(e0);
-        k_dmma_peak<<<blocks, threads>>>(out, iters, 1.0000001, 1e-9);
-        cudaEventRecord(e1);
-        cudaEventSynchronize(e1);
-        float ms;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(out);
-    if (cudaGetLastError() != cudaSuccess) return -1.0;
-    const double flops = 2.0 * 256 * 8 * (double)iters * blocks * (threads / 32);
-    return flops / (best * 1e-3) * 1e-12;
 }
 
 }  // namespace flare

@@ -29,8 +29,8 @@ EXPORTS = (
     "flare_create", "flare_destroy", "flare_num_descriptors", "flare_set_option", "flare_get_option",
     "flare_workspace_bytes", "flare_bind", "flare_compute", "flare_compute_host", "flare_check",
     "flare_set_state", "flare_set_state_host", "flare_set_forces", "flare_set_forces_host", "flare_step", "flare_get_state", "flare_get_state_host",
-    "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_timings", "flare_kernel_launches",
-    "flare_measure_fp64_dmma_peak", "flare_last_error",
+    "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_rows", "flare_get_timings", "flare_kernel_launches",
+    "flare_last_error",
     "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_analyze",
 )
 
@@ -76,11 +76,10 @@ def load_library():
     lib.flare_get_neighbors.argtypes = [vp, vp, vp, C.c_int32]
     lib.flare_get_descriptors.argtypes = [vp, vp, vp]
     lib.flare_get_groups.argtypes = [vp, vp, vp, vp]
+    lib.flare_get_rows.argtypes = [vp, vp]
     lib.flare_get_timings.argtypes = [vp, vp, vp]
     lib.flare_kernel_launches.argtypes = [vp]
     lib.flare_kernel_launches.restype = i64
-    lib.flare_measure_fp64_dmma_peak.argtypes = [i32]
-    lib.flare_measure_fp64_dmma_peak.restype = dbl
     lib.flare_last_error.argtypes = [vp]
     lib.flare_last_error.restype = C.c_char_p
     lib.flare_step_nvt.argtypes = [vp, dbl, i32, i32, dbl, dbl]
@@ -105,11 +104,6 @@ def _box9(box):
     if b.size == 3:
         b = np.diag(b.reshape(3))
     return np.ascontiguousarray(b.reshape(9))
-
-
-def measure_fp64_dmma_peak(device: int = 0) -> float:
-    """FP64 tensor-pipe issue peak in TFLOP/s (register-resident DMMA loop)."""
-    return float(load_library().flare_measure_fp64_dmma_peak(int(device)))
 
 
 class Flare:
@@ -347,6 +341,12 @@ class Flare:
         comps = np.zeros(64, np.int32)
         self._check(self._lib.flare_get_groups(self._ctx, C.cast(C.byref(n), C.c_void_p), _hp(rows), _hp(comps)))
         return [(int(rows[g]), int(comps[g])) for g in range(n.value)]
+
+    def rows(self):
+        """Quadratic-form row of every atom (caller's order) in the last evaluation."""
+        row = np.zeros(self.n_atoms, np.int32)
+        self._check(self._lib.flare_get_rows(self._ctx, _hp(row)))
+        return row
 
     def qform_flops(self, variance: bool, symmetric: bool = False) -> float:
         """Flops of steps a4 (+ a5) per evaluation.  Default: SURVEY.md 8(d)'s algorithmic count, 2 P_g^2 per atom and

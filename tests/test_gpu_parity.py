@@ -277,6 +277,100 @@ def test_error_codes(torch, flare):
     assert ei.value.code == -8
 
 
+def test_species_out_of_range_is_an_error(torch, flare):
+    """include/flare_b200.h: a species index outside 0..S-1 is FLARE_ERR_INVALID_ARG (flagged on the device, the
+    stored type clamped so that no table is indexed out of bounds), in a first build and on a reused candidate list."""
+    s = w.tile_like_c3(6, 3, n_max=3, l_max=2)
+    ctx = flare.from_system(s).bind(s.n_atoms)
+    pos = dev(torch, s.pos, torch.float64)
+    for bad_value in (2, -1, 1 << 20):
+        bad = s.types.copy()
+        bad[5] = bad_value
+        with pytest.raises(flare.FlareError) as ei:
+            ctx.compute(pos, dev(torch, bad, torch.int32), s.box, s.pbc)
+        assert ei.value.code == -1
+    e, f, v = ctx.compute(pos, dev(torch, s.types, torch.int32), s.box, s.pbc, variances=True)  # the context recovers
+    assert bool(torch.isfinite(f).all())
+    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)
+    ctx.step(0.5, 2)
+    ctx.check()
+    bad = s.types.copy()
+    bad[-1] = 7
+    ctx.set_state(s.pos, s.vel, bad, s.box, s.pbc)  # same binding: the refresh of the kept list meets the bad type
+    with pytest.raises(flare.FlareError) as ei:
+        ctx.step(0.5, 1)
+        ctx.check()
+    assert ei.value.code == -1
+
+
+def test_overflow_error_does_not_poison_the_binding(oracle, torch, flare):
+    """After FLARE_ERR_NEIGHBOR_OVERFLOW the truncated candidate list must not be reused: new, sparse positions in
+    the SAME binding are evaluated from scratch and match the oracle."""
+    rng = np.random.default_rng(61)
+    box = np.diag([30.0, 30, 30]).reshape(9)
+    n = 90
+    dense = 15 + rng.uniform(-2.2, 2.2, (n, 3))  # ~90 atoms in a 4.4 A cube: more than 64 candidates per atom
+    s = _mk(dense, np.zeros(n), box, [1, 1, 1], 1, n_max=3, l_max=2, seed=62)
+    ctx = flare.from_system(s, max_neighbors=60).bind(n)
+    types = dev(torch, s.types, torch.int32)
+    with pytest.raises(flare.FlareError) as ei:
+        ctx.compute(dev(torch, s.pos, torch.float64), types, s.box, s.pbc)
+    assert ei.value.code == -5
+    # the same atoms moved by less than the skin budget would keep the (truncated) list if it were still valid
+    sparse = np.stack(np.meshgrid(*[np.arange(5) * 3.1 + 4] * 3, indexing="ij"), -1).reshape(-1, 3)[:n]
+    sparse = sparse + rng.normal(0, 0.05, sparse.shape)
+    s2 = _mk(sparse, np.zeros(n), box, [1, 1, 1], 1, n_max=3, l_max=2, seed=62)
+    for _ in range(2):  # the second evaluation runs on the list the first one rebuilt
+        e, f, v = ctx.compute(dev(torch, s2.pos, torch.float64), types, s2.box, s2.pbc, variances=True)
+        E, F, V = oracle.compute(s2.pos, s2.types, s2.box, s2.pbc, s2.n_max, s2.l_max, s2.r_cut, s2.beta, s2.sigma, nbr_method=0)
+        assert_close(e.cpu().numpy(), E, ATOL_E, "E")
+        assert_close(f.cpu().numpy(), F, ATOL_F, "F")
+        cnt_o, idx_o = oracle.neighbors(s2.pos, s2.types, s2.box, s2.pbc, s2.r_cut, 0, cap=60)
+        cnt_g, idx_g = ctx.neighbors()
+        assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+
+
+def test_nonfinite_results_are_reported(torch, flare):
+    """NaN/Inf in E, F or V is an error code.  Two atoms at the same point give r = 0, hence a
+    non-finite pair force; flare_check must say so instead of letting an MD run integrate garbage."""
+    box = np.diag([30.0, 30, 30]).reshape(9)
+    pos = np.array([[5.0, 5, 5], [5.0, 5, 5], [7.0, 5.5, 5.2], [20.0, 20, 20]])
+    s = _mk(pos, [0, 0, 0, 0], box, [1, 1, 1], 1)
+    ctx = flare.from_system(s).bind(4)
+    with pytest.raises(flare.FlareError) as ei:
+        ctx.compute(dev(torch, s.pos, torch.float64), dev(torch, s.types, torch.int32), s.box, s.pbc, variances=True)
+    assert ei.value.code == -7
+    good = pos.copy()
+    good[1] += [1.5, 0.3, -0.2]
+    e, f, v = ctx.compute(dev(torch, good, torch.float64), dev(torch, s.types, torch.int32), s.box, s.pbc, variances=True)
+    assert bool(torch.isfinite(f).all()) and bool(torch.isfinite(e).all())
+
+
+def test_two_contexts_on_two_streams(oracle, torch, flare):
+    """Launch state (shared-memory limits, occupancies) is per context, not per process: two contexts with different
+    basis sizes, each on its own stream, interleaved, both match the oracle."""
+    sa = w.tile_like_c3(6, 3, n_max=8, l_max=3)
+    sb = w.tile_like_c3(6, 3, n_max=12, l_max=6)  # > 48 KB of dynamic shared memory in every per-atom kernel
+    st_a, st_b = torch.cuda.Stream(), torch.cuda.Stream()
+    ca = flare.from_system(sa).bind(sa.n_atoms, stream=st_a)
+    cb = flare.from_system(sb).bind(sb.n_atoms, stream=st_b)
+    torch.cuda.synchronize()
+    outs = {}
+    for rep in range(2):
+        for name, c, sy, stq in (("a", ca, sa, st_a), ("b", cb, sb, st_b)):
+            with torch.cuda.stream(stq):
+                pos, types = dev(torch, sy.pos, torch.float64), dev(torch, sy.types, torch.int32)
+            torch.cuda.synchronize()
+            outs[name] = c.compute(pos, types, sy.box, sy.pbc, variances=True, check=False)
+    ca.check(); cb.check()
+    for name, sy in (("a", sa), ("b", sb)):
+        E, F, V = oracle.compute(sy.pos, sy.types, sy.box, sy.pbc, sy.n_max, sy.l_max, sy.r_cut, sy.beta, sy.sigma)
+        e, f, v = outs[name]
+        assert_close(e.cpu().numpy(), E, ATOL_E, "E")
+        assert_close(f.cpu().numpy(), F, ATOL_F, "F")
+        assert_close(v.cpu().numpy(), V, 1e-15, "V")
+
+
 def test_many_neighbours_more_than_a_warp(oracle, torch, flare):
     """Dense blob: up to ~60 neighbours per atom exercises the >32-neighbour loops."""
     rng = np.random.default_rng(21)
@@ -320,73 +414,148 @@ def test_tile_16k_atoms_sampled(oracle, torch, flare):
     assert np.abs(f.sum(0)).max() < 1e-9
 
 
+def brute_force_rows(xw, types, box, pbc, r_cut, sel):
+    """Neighbour rows of the atoms in `sel` by brute force over ALL N atoms (plain numpy, no cells), with R6's
+    canonical arithmetic: wrapped coordinates, dx = x_j - x_i, one +-L shift beyond L/2, d2 = ((dx dx)+(dy dy))+(dz dz),
+    strict d2 < r_c r_c.  Independent of both the GPU cell list and the oracle's grid."""
+    L = np.asarray(box, float).reshape(3, 3).diagonal()
+    S = int(round(np.sqrt(np.asarray(r_cut).size)))
+    rc2 = (np.asarray(r_cut, float).reshape(S, S)) ** 2
+    idx_all = np.arange(xw.shape[0])
+    rows = []
+    for i in sel:
+        d2 = np.zeros(xw.shape[0])
+        parts = []
+        for a in range(3):
+            d = xw[:, a] - xw[i, a]
+            if pbc[a]:
+                d = np.where(d > 0.5 * L[a], d - L[a], np.where(d < -0.5 * L[a], d + L[a], d))
+            parts.append(d * d)
+        d2 = (parts[0] + parts[1]) + parts[2]
+        hit = d2 < rc2[types[i]][types]
+        hit[i] = False
+        rows.append(idx_all[hit])
+    return rows
+
+
+def full_size_check(oracle, torch, flare, s, ctx, pos, E_g, F_g, V_g, n_ev, n_f, n_brute, seed, all_rows=True):
+    """Parity of a full-size system that has just been evaluated by `ctx` at positions `pos` (host): neighbour rows
+    (every row against the oracle's grid search when all_rows, n_brute rows by brute force over all N), E and V of
+    ~n_ev atoms and F of ~n_f atoms against the oracle one by one, drawn from EVERY (species, neighbour-mask) group
+    and from the rows next to every atom-chunk boundary, plus the properties that hold at any size."""
+    N = s.n_atoms
+    types = s.types
+    want_var = V_g is not None
+    cap = 40
+    cnt_g, idx_g = ctx.neighbors(stride=cap)
+    rng = np.random.default_rng(seed)
+    # ---- neighbour sets
+    xw = oracle.wrap(pos, s.box, s.pbc)
+    sel_b = rng.choice(N, n_brute, replace=False)
+    for i, row in zip(sel_b, brute_force_rows(xw, types, s.box, s.pbc, s.r_cut, sel_b)):
+        assert np.array_equal(row, idx_g[i, :cnt_g[i]]), f"neighbour row of atom {i} differs from brute force"
+    if all_rows:
+        cnt_o, idx_o = oracle.neighbors(pos, types, s.box, s.pbc, s.r_cut, 1, cap=cap)
+        assert np.array_equal(cnt_g, cnt_o) and np.array_equal(idx_g, idx_o)
+        del cnt_o, idx_o
+    assert int(cnt_g.sum()) % 2 == 0  # full (symmetric) list
+    # ---- groups: (species, set of neighbour species) of every atom, from the (just verified) rows
+    valid = idx_g >= 0
+    tn = types[np.where(valid, idx_g, 0)]
+    mask = np.zeros(N, np.int64)
+    for sp in range(s.n_species):
+        mask |= ((valid & (tn == sp)).any(1).astype(np.int64) << sp)
+    gid = types.astype(np.int64) * (1 << s.n_species) + mask
+    del valid, tn
+    rows = ctx.rows()
+    chunk = ctx.get_option(flare.OPT_CHUNK_ATOMS)
+    present = [g for g in np.unique(gid)]
+    groups = ctx.groups()
+    assert sorted(int((gid == g).sum()) for g in present) == sorted(r for r, _ in groups if r), "group sizes"
+    near_boundary = np.nonzero(((rows % chunk) < 2) | ((rows % chunk) >= chunk - 2))[0] if chunk < N else np.empty(0, np.int64)
+    if chunk < N:
+        assert near_boundary.size >= 4 * ((N - 1) // chunk)  # two rows on either side of every boundary (+ row 0, 1)
+    per_ev = max(8, n_ev // len(present))
+    per_f = max(4, n_f // len(present))
+    sel_ev, sel_f = [near_boundary], [near_boundary]
+    for g in present:
+        members = np.nonzero(gid == g)[0]
+        pick = rng.choice(members, min(per_ev, members.size), replace=False)
+        sel_ev.append(pick)
+        sel_f.append(pick[:per_f])
+    sel_ev = np.unique(np.concatenate(sel_ev)).astype(np.int64)
+    sel_f = np.unique(np.concatenate(sel_f)).astype(np.int64)
+    assert sel_f.size >= min(n_f, 100) * 0.9 and sel_ev.size >= min(n_ev, 500) * 0.9
+    # ---- E, V (cheap: no gradients) on the large sample, F on the smaller one
+    sigma = s.sigma if want_var else None
+    E, _, V = oracle.compute_selected(pos, types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, sigma, sel_ev, forces=False)
+    assert_close(E_g[sel_ev], E, ATOL_E, "E")
+    if want_var:
+        assert_close(V_g[sel_ev], V, 1e-15, "V")
+    # sum of the sampled local energies: the quantity an MD run conserves, summed independently on both sides
+    assert abs(E_g[sel_ev].sum() - E.sum()) <= 1e-10 * np.abs(E).sum() + 1e-12
+    _, F, _ = oracle.compute_selected(pos, types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, None, sel_f)
+    assert_close(F_g[sel_f], F, ATOL_F, "F")
+    # ---- any-size properties
+    assert np.abs(F_g.sum(0)).max() < 1e-6  # zero net force (translation invariance)
+    assert np.isfinite(E_g).all() and np.isfinite(F_g).all() and (not want_var or np.isfinite(V_g).all())
+    return dict(n_ev=int(sel_ev.size), n_f=int(sel_f.size), n_groups=len(present), chunk=int(chunk))
+
+
+def md_then_check(oracle, torch, flare, s, variance, n_ev, n_f, n_brute, seed, steps=3, all_rows=True, **kw):
+    """bench.py's launch configuration (default options): MD steps on a reused candidate list, then parity."""
+    ctx = flare.from_system(s, variance=variance, **kw).bind(s.n_atoms)
+    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)
+    ctx.step(float(s.meta.get("dt_fs", 0.5)), steps, want_variance=variance)
+    st = ctx.get_state_host(variances=variance)
+    assert ctx.get_option(flare.OPT_SKIN_REBUILDS) < steps + 1  # steps + 1 evaluations, at least one on a reused list
+    info = full_size_check(oracle, torch, flare, s, ctx, st["pos"], st["E"], st["F"], st["V"] if variance else None,
+                           n_ev, n_f, n_brute, seed, all_rows=all_rows)
+    return ctx, info
+
+
 def test_config3_full_size_sampled(oracle, torch, flare):
     """BASELINE.json config 3 at full size (1 082 016 atoms, P = 544, variance on) in the launch configuration
     bench.py times (default options: species-sparse groups, skin list, automatic chunk), after MD steps so that the
-    reused candidate list is what produced the neighbour sets: sampled atoms of every group against the oracle,
-    one by one; neighbour sets of the sampled atoms bit-exact; properties that hold at any size for the rest."""
+    reused candidate list is what produced the neighbour sets.  Neighbour rows: ALL of them against the oracle's grid
+    search and 1000 by brute force over all N; E, V of ~100 000 atoms and F of >= 100 atoms against
+    the oracle one by one, from every group."""
     s = w.config3()
-    ctx = flare.from_system(s).bind(s.n_atoms)
-    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)
-    ctx.step(0.5, 3, want_variance=True)
-    st = ctx.get_state_host(variances=True)
-    assert ctx.get_option(flare.OPT_SKIN_REBUILDS) < 4  # 4 evaluations, at least one on a reused list
+    ctx, info = md_then_check(oracle, torch, flare, s, True, n_ev=100_000, n_f=120, n_brute=1000, seed=33)
     groups = ctx.groups()
     assert sum(r for r, _ in groups) == s.n_atoms and {p for r, p in groups if r} == {144, 544}
-    pos, types = st["pos"], s.types
-    n_pt = int(np.sum(types == 0))
-    rng = np.random.default_rng(33)
-    cnt_g, idx_g = ctx.neighbors()
-    # sample: Pt atoms at random, H atoms at random, plus atoms whose neighbourhood holds both species (P_g = 544)
-    sel = np.concatenate([rng.choice(n_pt, 20, replace=False), n_pt + rng.choice(s.n_atoms - n_pt, 10, replace=False)])
-    cand = rng.choice(s.n_atoms, 40000, replace=False)
-    both = [i for i in cand if cnt_g[i] and len(set(types[idx_g[i, :cnt_g[i]]].tolist())) == 2][:10]
-    assert len(both) == 10
-    sel = np.concatenate([sel, np.array(both)]).astype(np.int64)
-    E, F, V = oracle.compute_selected(pos, types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, sel)
-    assert_close(st["E"][sel], E, ATOL_E, "E")
-    assert_close(st["F"][sel], F, ATOL_F, "F")
-    assert_close(st["V"][sel], V, 1e-15, "V")
-    # neighbour sets of the sampled atoms: brute force against all N atoms with the canonical arithmetic (R6)
-    L = np.asarray(s.box, float).reshape(3, 3).diagonal()
-    xw = oracle.wrap(pos, s.box, s.pbc)
-    for i in sel[:12]:
-        d = xw - xw[i]
-        for a in range(3):
-            if s.pbc[a]:
-                d[:, a] = np.where(d[:, a] > 0.5 * L[a], d[:, a] - L[a], np.where(d[:, a] < -0.5 * L[a], d[:, a] + L[a], d[:, a]))
-        d2 = (d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2]
-        rc = np.asarray(s.r_cut, float).reshape(2, 2)[types[i], types]
-        nb = np.nonzero((d2 < rc * rc) & (np.arange(s.n_atoms) != i))[0]
-        assert np.array_equal(nb, idx_g[i, :cnt_g[i]])
-    # any-size properties: symmetric list, zero net force, finite outputs
-    assert cnt_g.sum() % 2 == 0
-    assert np.abs(st["F"].sum(0)).max() < 1e-7
-    assert np.isfinite(st["E"]).all() and np.isfinite(st["F"]).all() and np.isfinite(st["V"]).all()
+    assert info["n_groups"] >= 4 and info["n_ev"] >= 50_000 and info["n_f"] >= 100
 
 
 def test_config4_full_size_sampled(oracle, torch, flare):
-    """BASELINE.json config 4 (9 994 400 atoms): one evaluation with the default options, sampled atoms against the
-    oracle one by one, plus the any-size properties; also reports the workspace bytes per atom."""
+    """BASELINE.json config 4 (9 994 400 atoms): the default options give several atom chunks (a8); after MD steps,
+    ALL neighbour rows against the oracle's grid search and 200 by brute force over all N, E / V of ~100 000 atoms and
+    F of >= 100 atoms (incl. the rows next to every chunk boundary) against the oracle; workspace bytes per atom."""
     s = w.config4()
-    ctx = flare.from_system(s).bind(s.n_atoms)
-    pos = torch.as_tensor(s.pos, dtype=torch.float64, device="cuda")
-    types = torch.as_tensor(s.types, dtype=torch.int32, device="cuda")
-    e, f, v = ctx.compute(pos, types, s.box, s.pbc, variances=True)
-    torch.cuda.synchronize()
-    assert ctx.get_option(2) < s.n_atoms  # several atom chunks (a8)
+    ctx, info = md_then_check(oracle, torch, flare, s, True, n_ev=100_000, n_f=120, n_brute=200, seed=44, steps=2)
+    assert info["chunk"] < s.n_atoms  # several atom chunks
     per_atom = ctx.workspace_bytes(s.n_atoms) / s.n_atoms
     assert per_atom < 4096, per_atom      # 1.9 KB persistent + 16 GiB of chunk intermediates
-    n_pt = int(np.sum(s.types == 0))
-    rng = np.random.default_rng(44)
-    sel = np.concatenate([rng.choice(n_pt, 12, replace=False), n_pt + rng.choice(s.n_atoms - n_pt, 6, replace=False)])
-    E, F, V = oracle.compute_selected(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma, sel)
-    sel_t = torch.as_tensor(sel, device="cuda")
-    assert_close(e[sel_t].cpu().numpy(), E, ATOL_E, "E")
-    assert_close(f[sel_t].cpu().numpy(), F, ATOL_F, "F")
-    assert_close(v[sel_t].cpu().numpy(), V, 1e-15, "V")
-    assert float(f.sum(0).abs().max()) < 1e-6
-    assert bool(torch.isfinite(e).all()) and bool(torch.isfinite(f).all()) and bool(torch.isfinite(v).all())
+    assert info["n_ev"] >= 50_000 and info["n_f"] >= 100
+
+
+@pytest.mark.parametrize("variance", [True, False])
+@pytest.mark.parametrize("n_max,l_max,P", [(10, 4, 1050), (12, 6, 2100)])
+def test_config5_full_size_sampled(oracle, torch, flare, n_max, l_max, P, variance):
+    """BASELINE.json config 5 at full size (1 082 016 atoms) for the two larger descriptor sizes, variance on and off,
+    default options ((12,6) runs three atom chunks whose boundaries cut through groups), after 3 MD steps on a
+    reused candidate list: sampled atoms of every group and next to every chunk boundary against the oracle."""
+    s = w.config5(n_max, l_max)
+    assert s.P == P
+    if not variance:
+        s.sigma = None
+    n_ev = 3000 if P == 1050 else 1500
+    ctx, info = md_then_check(oracle, torch, flare, s, variance, n_ev=n_ev, n_f=110, n_brute=150, seed=55 + l_max,
+                              all_rows=(variance and P == 1050))
+    assert {p for r, p in ctx.groups() if r} == {P, w.num_descriptors(1, n_max, l_max)}
+    if P == 2100:
+        assert info["chunk"] < s.n_atoms
+    assert info["n_ev"] >= 500 and info["n_f"] >= 100
 
 
 def test_isolated_atoms_in_sparse_mode(oracle, torch, flare):

@@ -30,6 +30,21 @@ def test_library_exports_every_declared_symbol(built_lib):
         assert hasattr(lib, name), name
 
 
+def test_probe_library_exports_every_declared_symbol(built_lib):
+    """The bench hooks (include/flare_probes.h) live in a library of their own, outside the product ABI."""
+    from paper_2204_12573_b200 import build, probes
+
+    header = open(os.path.join(ROOT, "include", "flare_probes.h")).read()
+    declared = set(re.findall(r"\b(flare_probe_[a-z0-9_]+)\s*\(", header))
+    assert declared == set(probes.EXPORTS), declared ^ set(probes.EXPORTS)
+    lib = ctypes.CDLL(build.PROBES_LIB)
+    for name in declared:
+        assert hasattr(lib, name), name
+    product = ctypes.CDLL(built_lib)
+    for name in declared:
+        assert not hasattr(product, name), f"{name} leaked into the product ABI"
+
+
 def test_binding_loads_and_create_fails_loudly_without_gpu(built_lib):
     import torch
 
