@@ -383,12 +383,14 @@ def sweep_entries(args, local, peaks, t_start):
     import torch
 
     out = []
-    plan = [("c1", True, 200, 20), ("c2", True, 100, 20)]
+    # (workload, variance, steps, warm-up, FLARE_OPT_GRAPH): configs 1 and 2 replayed from the captured step (the
+    # default for small systems) and, for the per-phase kernel timeline, on plain launches
+    plan = [("c1", True, 400, 20, None), ("c1", True, 200, 20, 0), ("c2", True, 200, 20, None), ("c2", True, 100, 20, 0)]
     if args.sweep == "full":
-        plan += [("c5a", True, 6, 3), ("c5a", False, 6, 3), ("c5b", True, 4, 3), ("c5b", False, 4, 3),
-                 ("c5c", True, 3, 3), ("c5c", False, 3, 3), ("c4", True, 4, 3)]
+        plan += [("c5a", True, 6, 3, None), ("c5a", False, 6, 3, None), ("c5b", True, 4, 3, None),
+                 ("c5b", False, 4, 3, None), ("c5c", True, 3, 3, None), ("c5c", False, 3, 3, None), ("c4", True, 4, 3, None)]
     cache = {}
-    for name, var, steps, warm in plan:
+    for name, var, steps, warm, graph in plan:
         if time.perf_counter() - t_start > args.sweep_budget:
             out.append({"workload": name, "variance": var, "skipped": f"sweep time budget of {args.sweep_budget:.0f} s used up"})
             continue
@@ -411,15 +413,18 @@ def sweep_entries(args, local, peaks, t_start):
                 if name in _C5:
                     cache["c5geo"] = s
                     cache[(name,)] = (s.beta, s.sigma)
-            ctx, res = time_workload(s, args, local, steps, warm, 1, var)
+            ctx, res = time_workload(s, args, local, steps, warm, 1, var, graph=graph)
             med = res["median"]
             ph = {k: v[0] / steps for k, v in med["phases"].items()}
             flops = ctx.qform_flops(var)
             entry = {"workload": desc, "name": name, "atoms": s.n_atoms, "P": s.P, "variance": var, "steps": steps,
                      "warmup": warm, "ms_per_step": res["ms_per_step"], "value": s.n_atoms / (res["ms_per_step"] * 1e-3),
-                     "unit": UNIT, "launches_per_step": med["launches"] / steps, "phases_ms_per_step": ph,
+                     "unit": UNIT, "launches_per_step": med["launches"] / steps,
+                     "graph_replay": bool(ctx.get_option(8) > 0),
+                     "phases_ms_per_step": ph if any(ph.values()) else None,  # replayed steps record no phase events
                      "skin_rebuilds_in_window": med["skin_rebuilds"],
                      "qform_frac_of_dmma_peak": (flops / (ph["qform"] * 1e-3) * 1e-12 / peaks["dmma"]) if ph["qform"] > 0 else None,
+                     "qform_flop_count": "SURVEY 8(d): 2 P_g^2 per atom and form; qform_frac_executed counts the DMMAs issued",
                      "qform_frac_executed": (ctx.qform_flops(var, symmetric=True) / (ph["qform"] * 1e-3) * 1e-12 / peaks["dmma"])
                      if ph["qform"] > 0 else None,
                      "chunk_atoms": ctx.get_option(2), "workspace_bytes_per_atom": ctx.workspace_bytes(s.n_atoms) / s.n_atoms}

@@ -69,6 +69,14 @@ enum {
                                     them since the last build.  Candidate rows hold at most 64 entries
                                     (more: FLARE_ERR_NEIGHBOR_OVERFLOW; lower the skin).  Costs 360 B/atom. */
     FLARE_OPT_SKIN_REBUILDS = 6,  /* read-only (flare_get_option, synchronises): candidate-list rebuilds since flare_bind */
+    FLARE_OPT_GRAPH = 7,          /* CUDA-graph replay of the MD step in flare_step / flare_step_nvt (small systems are bound by launch
+                                    latency: one step of 256 atoms is ~30 tiny kernels).  -1 (default): automatic, for
+                                    n_atoms <= 200 000; 0: never; 1: always.  The first step of a run (and the step after a
+                                    re-bind, an option change or a new box) is launched plainly, the next one is captured
+                                    -- with the candidate-list rebuild chain as a conditional IF node that a device-side
+                                    decision switches on -- and later steps replay the graph on the bound stream.
+                                    Results are bit-identical to plain launches.  Replayed steps record no phase timings. */
+    FLARE_OPT_GRAPH_REPLAYS = 8,  /* read-only: steps replayed from the graph since flare_create */
     FLARE_OPT_SPECIES_SPARSE = 4 /* 1 (default when S * 2^S <= 64): atoms are grouped by the set of neighbour species
                                     present and the descriptor blocks of absent species are skipped in a2-a6
                                     ("420 to 112"); exact.  0: every atom uses all P components. */
@@ -232,7 +240,8 @@ int flare_get_rows(flare_ctx* ctx, int32_t* row);
  */
 int flare_get_timings(flare_ctx* ctx, double* ms, int64_t* launches);
 
-/* Number of kernels the library has launched on this context since creation. */
+/* Number of kernels the library has launched on this context since creation (steps replayed from a CUDA graph count
+   the kernels of the captured step; those of its conditional rebuild chain, which run only on demand, are left out). */
 int64_t flare_kernel_launches(const flare_ctx* ctx);
 
 const char* flare_last_error(const flare_ctx* ctx);

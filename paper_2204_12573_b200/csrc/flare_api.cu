@@ -77,6 +77,22 @@ struct flare_ctx {
     // bookkeeping
     int64_t launches = 0;
     LaunchCache launch_cache;  // per-context (= per-device) kernel attributes and occupancies
+    // CUDA graph of one MD step (small systems: the step is launch-latency bound)
+    int graph_opt = -1;                 // FLARE_OPT_GRAPH: -1 automatic, 0 never, 1 always
+    cudaStream_t cap_stream = nullptr;  // capture happens on library-owned streams (the bound one may be the legacy
+    cudaStream_t body_stream = nullptr; // default stream, which cannot be captured); replay goes to the bound stream
+    cudaGraph_t step_graph = nullptr;
+    cudaGraphExec_t step_exec = nullptr;
+    struct StepKey {
+        double dt = 0.0, T = 0.0, tau = 0.0;
+        int var = 0;
+        bool operator==(const StepKey& o) const { return dt == o.dt && T == o.T && tau == o.tau && var == o.var; }
+    } graph_key, plain_key;
+    bool plain_stepped = false;         // a plain (uncaptured) step with plain_key has run since the last invalidation
+    bool graph_broken = false;          // capture failed once: stay on plain launches
+    bool capturing = false;
+    int64_t graph_launches = 0;         // kernels per replay
+    int64_t graph_replays = 0;
     PhaseEvents phases[FLARE_N_PHASES];
     std::string err;
 };
@@ -89,6 +105,15 @@ Launcher make_launcher(flare_ctx* c) {
     L.launch_count = &c->launches;
     L.cache = &c->launch_cache;
     return L;
+}
+
+// the captured step bakes in pointers, the grid, options and dt: anything that changes them drops it
+void drop_step_graph(flare_ctx* c) {
+    if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
+    if (c->step_graph) cudaGraphDestroy(c->step_graph);
+    c->step_exec = nullptr;
+    c->step_graph = nullptr;
+    c->plain_stepped = false;
 }
 
 int fail(flare_ctx* c, int code, const std::string& msg) {
@@ -111,7 +136,7 @@ struct PhaseScope {
     int phase;
     int64_t l0;
     PhaseScope(flare_ctx* ctx, int p) : c(ctx), phase(p), l0(ctx->launches) {
-        if (!c->timing) return;
+        if (!c->timing || c->capturing) return;
         PhaseEvents& pe = c->phases[phase];
         if (pe.used == pe.start.size()) {
             cudaEvent_t a, b;
@@ -123,7 +148,7 @@ struct PhaseScope {
         cudaEventRecord(pe.start[pe.used], c->stream);
     }
     ~PhaseScope() {
-        if (!c->timing) return;
+        if (!c->timing || c->capturing) return;
         PhaseEvents& pe = c->phases[phase];
         cudaEventRecord(pe.stop[pe.used], c->stream);
         pe.used++;
@@ -325,6 +350,9 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
 // ---------------------------------------------------------------- box -> cell grid (R7)
 int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
     if (!box || !pbc) return fail(c, FLARE_ERR_INVALID_ARG, "box/pbc is null");
+    if (c->have_grid && memcmp(c->box, box, sizeof(double) * 9) == 0 && c->pbc[0] == (pbc[0] ? 1 : 0) &&
+        c->pbc[1] == (pbc[1] ? 1 : 0) && c->pbc[2] == (pbc[2] ? 1 : 0))
+        return FLARE_OK;  // same cell as before: the grid (and whatever was built on it) stands
     for (int i = 0; i < 9; i++)
         if (!std::isfinite(box[i])) return fail(c, FLARE_ERR_INVALID_ARG, "box has a non-finite entry");
     if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0)
@@ -357,7 +385,7 @@ int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
     g.stride[g.slow0] = g.nc[g.fast];
     g.stride[g.slow1] = g.nc[g.fast] * g.nc[g.slow0];
     g.n_cells = g.nc[0] * g.nc[1] * g.nc[2];
-    if (!c->have_grid || memcmp(&c->grid, &g, sizeof(Grid)) != 0) c->list_valid = false;  // new box: new list
+    if (!c->have_grid || memcmp(&c->grid, &g, sizeof(Grid)) != 0) { c->list_valid = false; drop_step_graph(c); }  // new box: new list
     c->grid = g;
     c->have_grid = true;
     memcpy(c->box, box, sizeof(double) * 9);
@@ -366,9 +394,9 @@ int setup_grid(flare_ctx* c, const double box[9], const int pbc[3]) {
 }
 
 // ---------------------------------------------------------------- one evaluation (steps a1-a8)
-int evaluate(flare_ctx* c, const double* pos, const int* types, double* e_out, double* f_out, double* var_out) {
+int evaluate(flare_ctx* c, Launcher& L, const double* pos, const int* types, double* e_out, double* f_out,
+             double* var_out) {
     const int n = (int)c->n;
-    Launcher L = make_launcher(c);
     const bool want_var = (var_out != nullptr) && c->has_sigma;
     if (var_out && !c->has_sigma) return fail(c, FLARE_ERR_INVALID_ARG, "variance requested but the model has no sigma");
     if (n == 0) return FLARE_OK;
@@ -482,6 +510,9 @@ int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_m
 void flare_destroy(flare_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
+    drop_step_graph(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->body_stream) cudaStreamDestroy(c->body_stream);
     for (void* p : c->dev_allocs) cudaFree(p);
     for (auto& pe : c->phases) {
         for (auto e : pe.start) cudaEventDestroy(e);
@@ -510,6 +541,12 @@ int flare_set_option(flare_ctx* c, int option, int64_t value) {
             if (value < 0 || value > 4000) return fail(c, FLARE_ERR_INVALID_ARG, "skin must be in 0..4000 (1e-3 Angstrom)");
             c->skin = 1e-3 * (double)value; c->n = -1;
             return FLARE_OK;
+        case FLARE_OPT_GRAPH:
+            if (value < -1 || value > 1) return fail(c, FLARE_ERR_INVALID_ARG, "graph option must be -1, 0 or 1");
+            c->graph_opt = (int)value;
+            c->graph_broken = false;
+            drop_step_graph(c);
+            return FLARE_OK;
         case FLARE_OPT_SPECIES_SPARSE:
             if (value && !c->have_sparse)
                 return fail(c, FLARE_ERR_UNSUPPORTED, "species-sparse mode needs S * 2^S <= 64 groups");
@@ -529,6 +566,8 @@ int flare_get_option(const flare_ctx* c, int option, int64_t* value) {
         case FLARE_OPT_TIMING: *value = c->timing; return FLARE_OK;
         case FLARE_OPT_SPECIES_SPARSE: *value = c->sparse; return FLARE_OK;
         case FLARE_OPT_SKIN_MILLI_ANGSTROM: *value = (int64_t)std::llround(c->skin * 1e3); return FLARE_OK;
+        case FLARE_OPT_GRAPH: *value = c->graph_opt; return FLARE_OK;
+        case FLARE_OPT_GRAPH_REPLAYS: *value = c->graph_replays; return FLARE_OK;
         case FLARE_OPT_SKIN_REBUILDS: {
             *value = 0;
             if (c->n >= 0 && c->ws.skin_gate) {
@@ -565,6 +604,7 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     c->have_grid = false;
     c->pairf_valid = false;
     c->list_valid = false;
+    drop_step_graph(c);
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.flags, 0, sizeof(int) * 4, c->stream));
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.scal, 0, sizeof(double) * 16, c->stream));  // thermostat xi = eta = 0
     if (c->ws.skin_gate) FLARE_CUDA(c, cudaMemsetAsync(c->ws.skin_gate, 0, sizeof(int) * 4, c->stream));
@@ -579,7 +619,8 @@ int flare_compute(flare_ctx* c, const double* pos, const int32_t* types, const d
     FLARE_CUDA(c, cudaSetDevice(c->device));
     rc = setup_grid(c, box, pbc);
     if (rc) return rc;
-    return evaluate(c, pos, types, e_out, f_out, var_out);
+    Launcher L = make_launcher(c);
+    return evaluate(c, L, pos, types, e_out, f_out, var_out);
 }
 
 int flare_check(flare_ctx* c) {
@@ -673,6 +714,71 @@ static int set_forces_impl(flare_ctx* c, const double* f, cudaMemcpyKind kind) {
 int flare_set_forces(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyDeviceToDevice); }
 int flare_set_forces_host(flare_ctx* c, const double* f) { return set_forces_impl(c, f, cudaMemcpyHostToDevice); }
 
+// one velocity-Verlet step (with T_kelvin > 0 bracketed by Nose-Hoover half steps, R19) enqueued through L
+static int enqueue_md_step(flare_ctx* c, Launcher& L, double dt_fs, double* var, bool nvt, double gkT, double Q) {
+    const int n = (int)c->n;
+    Workspace& w = c->ws;
+    {
+        PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
+        if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
+        run_kick_drift(L, c->grid, n, w.x, w.v, w.f, w.types, c->d_accel, dt_fs);
+    }
+    int rc = evaluate(c, L, w.x, w.types, w.e, w.f, var);
+    if (rc) return rc;
+    {
+        PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
+        run_kick(L, n, w.v, w.f, w.types, c->d_accel);
+        if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
+    }
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "integrator launch");
+    return FLARE_OK;
+}
+
+// Small systems are bound by launch latency, not by the GPU (a 256-atom step is ~30 tiny kernels): capture one whole
+// MD step -- integrator, neighbour phase with the rebuild chain as a conditional IF node, descriptors, quadratic
+// forms, back-propagation, gather -- into a CUDA graph once and replay it ("saturated
+// performance ... for small systems").  The launch sequence of a step on a kept candidate list is static, and the
+// decision to rebuild is taken on the device, so one graph serves every step of a run.
+static bool graph_wanted(const flare_ctx* c) {
+    if (c->graph_broken || c->graph_opt == 0 || c->n <= 0) return false;
+    if (c->graph_opt == 1) return true;
+    return c->n <= 200000;  // automatic: above this a step keeps the GPU busy for longer than its launches take
+}
+
+static int capture_md_step(flare_ctx* c, double dt_fs, double* var, bool nvt, double gkT, double Q) {
+    if (!c->cap_stream) {
+        FLARE_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+        FLARE_CUDA(c, cudaStreamCreateWithFlags(&c->body_stream, cudaStreamNonBlocking));
+    }
+    drop_step_graph(c);
+    FLARE_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    Launcher L = make_launcher(c);
+    L.stream = c->cap_stream;
+    L.body_stream = c->body_stream;
+    L.capturing = true;
+    c->capturing = true;
+    const int64_t l0 = c->launches;
+    int rc = enqueue_md_step(c, L, dt_fs, var, nvt, gkT, Q);
+    c->capturing = false;
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    c->graph_launches = c->launches - l0;
+    c->launches = l0;  // nothing has run yet; replays add their launches
+    if (rc == FLARE_OK && e != cudaSuccess) rc = cuda_fail(c, e, "cudaStreamEndCapture");
+    if (rc == FLARE_OK) {
+        e = cudaGraphInstantiate(&c->step_exec, g, 0);
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "cudaGraphInstantiate");
+    }
+    if (rc != FLARE_OK) {
+        if (g) cudaGraphDestroy(g);
+        c->step_exec = nullptr;
+        cudaGetLastError();
+        return rc;
+    }
+    c->step_graph = g;
+    return FLARE_OK;
+}
+
 // velocity Verlet; with T_kelvin > 0 each step is bracketed by Nose-Hoover half steps (R19)
 static int step_impl(flare_ctx* c, double dt_fs, int n_steps, int want_variance, double T_kelvin, double tau_fs) {
     int rc = need_bound(c);
@@ -684,8 +790,9 @@ static int step_impl(flare_ctx* c, double dt_fs, int n_steps, int want_variance,
     const int n = (int)c->n;
     Workspace& w = c->ws;
     double* var = want_variance ? w.var : nullptr;
+    Launcher L = make_launcher(c);
     if (!c->forces_valid || (want_variance && !c->var_valid && n_steps == 0)) {
-        rc = evaluate(c, w.x, w.types, w.e, w.f, var);
+        rc = evaluate(c, L, w.x, w.types, w.e, w.f, var);
         if (rc) return rc;
         c->forces_valid = true;
         c->var_valid = want_variance != 0;
@@ -699,26 +806,34 @@ static int step_impl(flare_ctx* c, double dt_fs, int n_steps, int want_variance,
                                       cudaMemcpyHostToDevice, c->stream));
         c->accel_dt = dt_fs;
     }
-    Launcher L = make_launcher(c);
     const bool nvt = T_kelvin > 0.0;
     const double gkT = (3.0 * (double)n - 3.0) * 8.617333262e-5 * T_kelvin;  // g k_B T, g = 3N - 3 (R13, R19)
     const double Q = gkT * tau_fs * tau_fs;
+    flare_ctx::StepKey key;
+    key.dt = dt_fs; key.T = nvt ? T_kelvin : 0.0; key.tau = nvt ? tau_fs : 0.0; key.var = want_variance ? 1 : 0;
     for (int step = 0; step < n_steps; step++) {
-        {
-            PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
-            if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
-            run_kick_drift(L, c->grid, n, w.x, w.v, w.f, w.types, c->d_accel, dt_fs);
+        // a step can be replayed from the graph when its launch sequence is the captured one: the candidate list is
+        // kept (or there is none), and a plain step with the same parameters has run (every kernel is loaded)
+        const bool static_chain = eff_skin(c) == 0.0 || c->list_valid;
+        if (graph_wanted(c) && static_chain && c->plain_stepped && c->plain_key == key) {
+            if (!c->step_exec || !(c->graph_key == key)) {
+                rc = capture_md_step(c, dt_fs, var, nvt, gkT, Q);
+                if (rc != FLARE_OK) { c->graph_broken = true; c->step_exec = nullptr; }
+                else c->graph_key = key;
+            }
+            if (c->step_exec) {
+                FLARE_CUDA(c, cudaGraphLaunch(c->step_exec, c->stream));
+                c->launches += c->graph_launches;
+                c->graph_replays++;
+                continue;
+            }
         }
-        rc = evaluate(c, w.x, w.types, w.e, w.f, var);
+        rc = enqueue_md_step(c, L, dt_fs, var, nvt, gkT, Q);
         if (rc) return rc;
-        {
-            PhaseScope ps(c, FLARE_PHASE_INTEGRATE);
-            run_kick(L, n, w.v, w.f, w.types, c->d_accel);
-            if (nvt) run_nh_half(L, w, n, c->d_mass, 0.5 * dt_fs, gkT, Q, w.scal + 12);
-        }
+        c->plain_stepped = true;
+        c->plain_key = key;
     }
     c->var_valid = want_variance != 0;
-    if (L.err != cudaSuccess) return cuda_fail(c, L.err, "integrator launch");
     return FLARE_OK;
 }
 

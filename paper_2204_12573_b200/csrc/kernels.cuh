@@ -63,7 +63,8 @@ struct Launcher {
     void launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
         if (grid.x == 0 || grid.y == 0 || grid.z == 0 || err != cudaSuccess) return;
         kernel<<<grid, block, smem, stream>>>(std::forward<Args>(args)...);
-        if (launch_count) ++*launch_count;
+        // kernels captured into a conditional IF body run only when the device switches the node on: not counted
+        if (launch_count && outer_stream == nullptr) ++*launch_count;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = "kernel launch"; }
     }
@@ -71,6 +72,59 @@ struct Launcher {
         if (bytes == 0 || err != cudaSuccess) return;
         cudaError_t e = cudaMemsetAsync(p, v, bytes, stream);
         if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = "memset"; }
+    }
+
+    // ---- CUDA-graph capture of the step (small systems, flare_api.cu): `stream` is being captured.  A conditional
+    // IF node lets the graph skip the whole candidate-list rebuild chain unless the device-side gate asks for it:
+    //   h = cond_handle();  launch(kernel that calls cudaGraphSetConditional(h, need));  begin_if(h);
+    //   ... launches of the body ...;  end_if();
+    bool capturing = false;
+    cudaStream_t body_stream = nullptr;  // side stream the IF body is captured on
+    cudaStream_t outer_stream = nullptr;
+    cudaGraphNode_t cond_node = nullptr;
+    void fail_here(cudaError_t e, const char* where) {
+        if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = where; }
+    }
+    cudaGraphConditionalHandle cond_handle() {
+        cudaGraphConditionalHandle h = 0;
+        if (err != cudaSuccess) return h;
+        cudaStreamCaptureStatus st;
+        cudaGraph_t g = nullptr;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t nd = 0;
+        fail_here(cudaStreamGetCaptureInfo_v2(stream, &st, nullptr, &g, &deps, &nd), "cudaStreamGetCaptureInfo");
+        if (err == cudaSuccess) fail_here(cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault), "cudaGraphConditionalHandleCreate");
+        return h;
+    }
+    void begin_if(cudaGraphConditionalHandle h) {
+        if (err != cudaSuccess) return;
+        cudaStreamCaptureStatus st;
+        cudaGraph_t g = nullptr;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t nd = 0;
+        fail_here(cudaStreamGetCaptureInfo_v2(stream, &st, nullptr, &g, &deps, &nd), "cudaStreamGetCaptureInfo");
+        if (err != cudaSuccess) return;
+        cudaGraphNodeParams p = {cudaGraphNodeTypeConditional};
+        p.conditional.handle = h;
+        p.conditional.type = cudaGraphCondTypeIf;
+        p.conditional.size = 1;
+        fail_here(cudaGraphAddNode(&cond_node, g, deps, nd, &p), "cudaGraphAddNode(conditional)");
+        if (err != cudaSuccess) return;
+        fail_here(cudaStreamBeginCaptureToGraph(body_stream, p.conditional.phGraph_out[0], nullptr, nullptr, 0,
+                                                cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCaptureToGraph");
+        if (err != cudaSuccess) return;
+        outer_stream = stream;
+        stream = body_stream;
+    }
+    void end_if() {
+        if (outer_stream == nullptr) return;
+        cudaError_t e = cudaStreamEndCapture(body_stream, nullptr);
+        stream = outer_stream;
+        outer_stream = nullptr;
+        fail_here(e, "cudaStreamEndCapture(conditional body)");
+        if (err == cudaSuccess)
+            fail_here(cudaStreamUpdateCaptureDependencies(stream, &cond_node, 1, cudaStreamSetCaptureDependencies),
+                      "cudaStreamUpdateCaptureDependencies");
     }
 };
 

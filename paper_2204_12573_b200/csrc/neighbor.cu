@@ -444,15 +444,18 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
 // d_a + d_b < (rc_max + skin) - r_cut[a][b]: the pairs with the largest cutoff have `skin` to spend, pairs with a
 // shorter cutoff (every pair with an H in the H2/Pt workloads) much more, so the fast light atoms do not force
 // rebuilds.  The threshold is taken a hair low so that the triangle inequality holds with rounding to spare.
-__global__ void k_gate_decide(Basis bs, double reach, const int* __restrict__ dmax, int* __restrict__ gate) {
+// In a captured step (CUDA graph, small systems) the decision also drives the IF node that holds the rebuild chain.
+__global__ void k_gate_decide(Basis bs, double reach, const int* __restrict__ dmax, int* __restrict__ gate,
+                              cudaGraphConditionalHandle cond, int use_cond) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    int need = 0;
+    int need = *gate;  // k_refresh raises it for a non-finite position or a changed species
     for (int a = 0; a < bs.S; a++)
         for (int b = a; b < bs.S; b++) {
             const double da = __int_as_float(dmax[a]), db = __int_as_float(dmax[b]);
             if (!(da + db < 0.9998 * (reach - bs.rc[a * bs.S + b]))) need = 1;
         }
     if (need) *gate = 1;
+    if (use_cond) cudaGraphSetConditional(cond, need ? 1u : 0u);
 }
 
 __global__ void k_copy_ref(int n, const AtomS* __restrict__ atoms, AtomS* __restrict__ ref, const int* __restrict__ gate,
@@ -668,7 +671,13 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
             L.memset(ws.skin_gate + 4, 0, sizeof(int) * kMaxSpecies);  // per-species maximum displacement
             L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, bs.S, n, pos, types, (const int*)ws.order,
                      (const AtomS*)ws.ref, ws.atoms, ws.skin_gate, ws.skin_gate + 4, ws.flags);
-            L.launch(k_gate_decide, dim3(1), dim3(32), 0, bs, reach, (const int*)(ws.skin_gate + 4), ws.skin_gate);
+            // captured step: the rebuild chain below becomes the body of an IF node that k_gate_decide switches on,
+            // so a step that keeps its list pays for none of the chain's (otherwise empty) launches
+            const bool as_if = L.capturing;
+            const cudaGraphConditionalHandle h = as_if ? L.cond_handle() : 0;
+            L.launch(k_gate_decide, dim3(1), dim3(32), 0, bs, reach, (const int*)(ws.skin_gate + 4), ws.skin_gate, h,
+                     as_if ? 1 : 0);
+            if (as_if) { L.begin_if(h); gate = nullptr; }
         }
     }
     L.memset(ws.cell_cnt, 0, sizeof(int) * (size_t)g.n_cells);
@@ -694,6 +703,7 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
              gate);
     if (use_skin) {
         L.launch(k_copy_ref, dim3((n + tb - 1) / tb), dim3(tb), 0, n, (const AtomS*)ws.atoms, ws.ref, gate, ws.skin_gate + 1);
+        L.end_if();  // no-op unless the chain was captured as an IF body
         const int nfb = (n + kNbrWarps * kFilterAtoms - 1) / (kNbrWarps * kFilterAtoms);
         L.launch(k_filter, dim3(nfb), dim3(kNbrWarps * 32), 0, g, bs, n, mmax, bmax, (const AtomS*)ws.atoms,
                  (const int*)ws.skin_cnt, (const int*)ws.skin_idx, ws.nbr_cnt, ws.nbr_idx, ws.nmask, ws.hitmask, ws.flags);

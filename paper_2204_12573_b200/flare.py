@@ -22,6 +22,7 @@ ERRORS = {
     -7: "FLARE_ERR_NONFINITE", -8: "FLARE_ERR_UNSUPPORTED", -9: "FLARE_ERR_NOT_BOUND",
 }
 OPT_MAX_NEIGHBORS, OPT_CHUNK_ATOMS, OPT_TIMING, OPT_SPECIES_SPARSE, OPT_SKIN, OPT_SKIN_REBUILDS = 1, 2, 3, 4, 5, 6
+OPT_GRAPH, OPT_GRAPH_REPLAYS = 7, 8
 PHASES = ("neighbor", "descriptor", "qform", "backprop", "gather", "integrate")
 
 # every symbol include/flare_b200.h declares (checked by the CPU test-suite)
@@ -111,7 +112,7 @@ class Flare:
 
     def __init__(self, mass, n_max: int, l_max: int, r_cut, beta, sigma=None, device: int = 0,
                  max_neighbors: int | None = None, chunk_atoms: int | None = None, timing: bool = False,
-                 species_sparse: bool | None = None, skin: float | None = None):
+                 species_sparse: bool | None = None, skin: float | None = None, graph: int | None = None):
         import torch  # device memory + stream only
 
         self._torch = torch
@@ -148,6 +149,8 @@ class Flare:
             self.set_option(OPT_SPECIES_SPARSE, 1 if species_sparse else 0)
         if skin is not None:
             self.set_option(OPT_SKIN, int(round(1e3 * skin)))  # Angstrom -> 1e-3 Angstrom
+        if graph is not None:
+            self.set_option(OPT_GRAPH, int(graph))  # -1 automatic, 0 never, 1 always
 
     # ------------------------------------------------------------------ plumbing
     def _check(self, rc: int):

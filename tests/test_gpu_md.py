@@ -219,3 +219,69 @@ def test_skin_list_edge_geometries(oracle, torch, flare, case):
         if s.pbc[a]:
             d[:, a] -= L3[a] * np.round(d[:, a] / L3[a])
     assert np.abs(d).max() < 1e-7
+
+
+# ----------------------------------------------------------------------------- CUDA-graph replay of the step (small systems)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2_hot", "c2_nvt", "c2_noskin"])
+def test_graph_replay_is_bit_identical_to_plain_launches(torch, flare, name):
+    """FLARE_OPT_GRAPH: a run replayed from the captured step (with the candidate-list rebuild chain as a conditional
+    IF node) gives bit for bit the trajectory of plain launches, across list rebuilds, for NVE and NVT, with and
+    without a candidate list; the graph is really used (replay counter) and dropped when dt changes."""
+    if name == "c1":
+        s, dt, steps = w.config1(), 1.0, 40
+    else:
+        s, dt, steps = w.config2(), 0.5, 60
+        if name == "c2_hot":  # hot gas: several rebuilds of the candidate list inside the run
+            s.vel = w.maxwell_velocities(np.random.default_rng(5), s.types, s.mass, 6000.0)
+    kw = dict(skin=0.0) if name == "c2_noskin" else {}
+    runs = {}
+    for graph in (0, 1):
+        ctx = start(torch, flare, s, graph=graph, **kw)
+        if name == "c2_nvt":
+            ctx.step_nvt(dt, steps, 500.0, 50.0, want_variance=True)
+            ctx.step_nvt(dt, 5, 500.0, 50.0, want_variance=True)
+        else:
+            ctx.step(dt, steps, want_variance=True)
+            ctx.step(dt, 5, want_variance=True)       # a second call keeps replaying
+            ctx.step(0.5 * dt, 4, want_variance=True)  # new dt: one plain step, a new capture, replays
+        st = ctx.get_state_host(variances=True)
+        runs[graph] = (st, ctx.get_option(flare.OPT_SKIN_REBUILDS), ctx.get_option(flare.OPT_GRAPH_REPLAYS),
+                       ctx.thermostat() if name == "c2_nvt" else None, ctx.kernel_launches())
+    (a, ra, pa, ta, la), (b, rb, pb, tb, lb) = runs[0], runs[1]
+    assert pa == 0 and pb >= steps + 5 - 1 - 1
+    for k in ("pos", "vel", "E", "F", "V"):
+        assert np.array_equal(a[k], b[k]), k
+    assert ra == rb and ta == tb
+    if name == "c2_hot":
+        assert rb >= 3, rb  # the IF body ran inside replayed steps
+    if name == "c2_noskin":
+        assert rb == 0
+    # a replayed step on a kept list launches fewer kernels than a plain one (the rebuild chain is skipped, not emptied)
+    if name in ("c1", "c2_nvt"):
+        assert lb < la
+
+
+def test_graph_option_automatic_threshold_and_off(torch, flare):
+    s = w.config1()
+    ctx = start(torch, flare, s)  # automatic: 256 atoms are far below the threshold
+    assert ctx.get_option(flare.OPT_GRAPH) == -1
+    ctx.step(1.0, 6)
+    assert ctx.get_option(flare.OPT_GRAPH_REPLAYS) == 5  # step 1 plain, step 2 captured + replayed, ...
+    ctx.set_option(flare.OPT_GRAPH, 0)
+    ctx.step(1.0, 3)
+    assert ctx.get_option(flare.OPT_GRAPH_REPLAYS) == 5
+    # an error inside a replayed run is still reported, and the run recovers on plain launches
+    bad = s.pos.copy()
+    bad[3] = np.nan
+    ctx.set_option(flare.OPT_GRAPH, 1)
+    ctx.step(1.0, 3)
+    ctx.set_state(bad, s.vel, s.types, s.box, s.pbc)
+    with pytest.raises(flare.FlareError) as ei:
+        ctx.step(1.0, 2)
+        ctx.check()
+    assert ei.value.code == -7
+    ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc)
+    ctx.step(1.0, 3)
+    ctx.check()
