@@ -751,6 +751,7 @@ static int capture_md_step(flare_ctx* c, double dt_fs, double* var, bool nvt, do
         FLARE_CUDA(c, cudaStreamCreateWithFlags(&c->body_stream, cudaStreamNonBlocking));
     }
     drop_step_graph(c);
+    c->plain_stepped = true;  // the caller checked it; dropping the OLD graph must not ask for another plain step
     FLARE_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
     Launcher L = make_launcher(c);
     L.stream = c->cap_stream;
