@@ -65,11 +65,10 @@ __device__ __forceinline__ double wrap_coord(double x, double L) {
 }
 
 __device__ __forceinline__ double min_image(double d, double L, double half, int pbc) {
-    if (pbc) {
-        if (d > half) d = __dsub_rn(d, L);
-        else if (d < -half) d = __dadd_rn(d, L);
-    }
-    return d;
+    // selects, not branches (same values: each candidate is one rounded operation on d)
+    const double lo = __dsub_rn(d, L), hi = __dadd_rn(d, L);
+    const double w = d > half ? lo : (d < -half ? hi : d);
+    return pbc ? w : d;
 }
 
 __device__ __forceinline__ double dist2_canonical(double dx, double dy, double dz) {

@@ -127,9 +127,14 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
         k = __shfl_sync(kFull, my_k, ai);
         s = p - __shfl_sync(kFull, my_start, ai);
     };
+    // pipeline depth 2: the neighbour INDEX of pass q+2 and the two ATOMS of pass q+1 are requested during pass q,
+    // so that neither the index -> atom dependency nor the atom loads themselves stall a pass
     int ai_n, k_n, s_n, j_n = 0;
     locate(lane, ai_n, k_n, s_n);
     if (lane < T) j_n = nbr_idx[(size_t)k_n * mmax + s_n];
+    int ai_nn, k_nn, s_nn, j_nn = 0;
+    locate(lane + 32, ai_nn, k_nn, s_nn);
+    if (lane + 32 < T) j_nn = nbr_idx[(size_t)k_nn * mmax + s_nn];
     AtomS me_n = load_atom(atoms + k_n), o_n = load_atom(atoms + j_n);
 
     // ---------------- phase 1: per atom E, V, c, G
@@ -238,10 +243,13 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
         const int ai = ai_n, k = k_n, s = s_n;
         const AtomS me = me_n, o = o_n;
         if (p0 + 32 < T) {  // uniform
-            locate(p + 32, ai_n, k_n, s_n);
-            j_n = (p + 32 < T) ? nbr_idx[(size_t)k_n * mmax + s_n] : 0;
+            ai_n = ai_nn; k_n = k_nn; s_n = s_nn; j_n = j_nn;
             me_n = load_atom(atoms + k_n);
             o_n = load_atom(atoms + j_n);
+            if (p0 + 64 < T) {  // uniform
+                locate(p + 64, ai_nn, k_nn, s_nn);
+                j_nn = (p + 64 < T) ? nbr_idx[(size_t)k_nn * mmax + s_nn] : 0;
+            }
         }
         if (p < T) {
             double dx, dy, dz;
@@ -294,8 +302,9 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
     // into each 32-lane pass, so take the largest count that still lets min(ctas1, 4) CTAs fit.
     int ta = kBpMaxTA;
     if (gr.nsp > 0) {
-        const size_t sm_bytes = 227 * 1024;
-        auto cta_bytes = [&](int t) { return sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(t, gr.nsp, Nc8, gr.K); };
+        const size_t sm_bytes = 228 * 1024;  // per SM
+        // + 1 KB: the shared memory the system reserves per resident CTA
+        auto cta_bytes = [&](int t) { return sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(t, gr.nsp, Nc8, gr.K) + 1024; };
         int target = (int)(sm_bytes / cta_bytes(1));
         target = target > 4 ? 4 : (target < 1 ? 1 : target);
         while (ta > 1 && cta_bytes(ta) * target > sm_bytes) ta--;
