@@ -47,7 +47,7 @@ enum {
     FLARE_ERR_INVALID_ARG = -1,        /* null pointer, bad size, species out of range, asymmetric r_cut (R5) */
     FLARE_ERR_BOX_TOO_SMALL = -2,      /* a periodic box length < 2 max r_cut: no unique minimum image (R7) */
     FLARE_ERR_UNSUPPORTED_BOX = -3,    /* non-orthorhombic cell (R7) */
-    FLARE_ERR_WORKSPACE_TOO_SMALL = -4,
+    FLARE_ERR_WORKSPACE_TOO_SMALL = -4, /* also: a domain-decomposition message, send list or capacity is too small */
     FLARE_ERR_NEIGHBOR_OVERFLOW = -5,  /* an atom has more than FLARE_OPT_MAX_NEIGHBORS neighbours */
     FLARE_ERR_CUDA = -6,               /* CUDA runtime error; message in flare_last_error */
     FLARE_ERR_NONFINITE = -7,          /* NaN/Inf met in positions, or produced in an energy, force or variance */
@@ -205,6 +205,75 @@ int flare_get_virial(flare_ctx* ctx, double virial[9]);
  */
 int flare_analyze(flare_ctx* ctx, double unc_threshold, int species_a, int species_b, double r_coord,
                   double* max_unc, int64_t* n_above, int32_t* coord, int64_t* coord_hist);
+
+/*
+ * ---- Multi-GPU: spatial domain decomposition with a halo exchange per step (what the paper gets from LAMMPS:
+ * P:L163 "MD runs entirely on GPUs with zero CPU-GPU data transfer except for I/O ... GPU-GPU communication";
+ * near-perfect weak scaling P:L239; "near-two-dimensional" geometry P:L233).  One process per GPU owns the atoms
+ * of one rectangle of a 2-D (x, y) process grid and evaluates them together with ghost copies of every atom within
+ * the halo width h >= 2 max r_cut + 2 * (trigger displacement) of the rectangle, so that the forces on owned atoms
+ * need no reverse exchange.  The library provides the DEVICE DATA PLANE: selection, packing, compaction and
+ * unpacking kernels and every count live on the device; the caller only moves the message buffers between ranks
+ * (e.g. NCCL send/recv) in the order below.  The state arrays of the context hold
+ *     [ owned atoms ][ ghosts received in phase 0 (from lo, from hi) ][ ghosts received in phase 1 ]
+ * in a LOCAL frame: a decomposed dimension is open (pbc = 0) with length w + 2 h and the owned rectangle at
+ * [h, h + w); the frame of the neighbour on the lo side is shifted by +w, on the hi side by -w, so periodic images
+ * need no special case.  Phase 0 exchanges along the first decomposed axis, phase 1 along the second and includes
+ * the ghosts of phase 0 (corners).  Bind the context with the CAPACITY (owned + ghosts + slack) as n_atoms.
+ *
+ * Messages are device arrays of doubles: [0] = number of rows, rows start at double 8.  A full row is
+ * (x, y, z, vx, vy, vz, fx, fy, fz, type, tag) = 11 doubles, a forward row (x, v, f) = 9 doubles; a message for
+ * cap_rows rows needs 8 + 11 cap_rows doubles.  Messages of a REBUILD travel at full capacity with the count in the
+ * header (no size round trip); forward messages have the sizes flare_domain_commit returned.
+ *
+ * Rebuild (every rank, same order):  [ per decomposed axis: migrate_pack -> exchange -> migrate_unpack ]
+ *     [ per phase: border_pack -> exchange -> border_unpack ]  commit.
+ * Step:  [ per phase: forward_pack -> exchange -> forward_unpack ]  flare_step(dt, 1, ...)  flare_domain_signal.
+ * Between two rebuilds membership, order and counts are fixed, so the candidate neighbour list of the context is
+ * kept (FLARE_OPT_SKIN_MILLI_ANGSTROM) and nothing blocks the host.  Ghosts carry their owner's velocity and force,
+ * so flare_step moves them exactly as their owner does.  All calls are asynchronous on the bound stream except
+ * flare_domain_begin and flare_domain_commit.  Too small a message, send list or capacity raises
+ * FLARE_ERR_WORKSPACE_TOO_SMALL at the next flare_check / flare_domain_commit.
+ */
+
+/* Start domain mode: the first n_owned atoms of the state become pos / vel (may be NULL = 0) / types / tags (global
+   atom ids, they travel with the atoms), all DEVICE pointers, in the local frame `box`, `pbc` (host).  A displacement
+   of any atom by trigger_displacement (Angstrom) since the last rebuild raises the rebuild signal (0: always raised). */
+int flare_domain_begin(flare_ctx* ctx, int64_t n_owned, const double* pos, const double* vel, const int32_t* types,
+                       const int64_t* tags, const double box[9], const int pbc[3], double trigger_displacement);
+
+/* Owned atoms with coordinate[axis] < lo_bound (>= hi_bound) leave through the lo (hi) face: their full rows, shifted
+   by shift_lo (shift_hi) along the axis, go to msg_lo (msg_hi); the atoms that stay are compacted in order.  Drops all
+   ghosts. */
+int flare_domain_migrate_pack(flare_ctx* ctx, int axis, double lo_bound, double hi_bound, double shift_lo,
+                              double shift_hi, double* msg_lo, double* msg_hi, int64_t cap_rows);
+/* Append the atoms of the two received messages (either may be NULL) to the owned set. */
+int flare_domain_migrate_unpack(flare_ctx* ctx, const double* msg_lo_in, const double* msg_hi_in, int64_t cap_rows);
+
+/* Phase 0 or 1: local atoms (owned, plus the ghosts of phase 0 in phase 1) with coordinate[axis] in [lo_a, lo_b)
+   form the send list towards the lo neighbour, those in [hi_a, hi_b) the one towards the hi neighbour; their full
+   rows (shifted) are packed.  The lists stay fixed until the next rebuild. */
+int flare_domain_border_pack(flare_ctx* ctx, int phase, int axis, double lo_a, double lo_b, double hi_a, double hi_b,
+                             double shift_lo, double shift_hi, double* msg_lo, double* msg_hi, int64_t cap_rows);
+/* Append the ghosts received from the lo neighbour, then from the hi neighbour (NULL: none) and remember their slots. */
+int flare_domain_border_unpack(flare_ctx* ctx, int phase, const double* msg_lo_in, const double* msg_hi_in,
+                               int64_t cap_rows);
+
+/* End of a rebuild (synchronises): the local atom count becomes the context's n_atoms, the candidate list is dropped,
+   the rebuild signal cleared.  counts (host, may be NULL): [0] local atoms, [1] owned, [2..5] rows of the forward
+   messages sent to x-lo, x-hi, y-lo, y-hi, [6..9] rows received from them, [10..13] their first slots. */
+int flare_domain_commit(flare_ctx* ctx, int64_t counts[14]);
+
+/* Per step: forward rows (x + shift, v, f) of the phase's two send lists -> messages; received rows -> ghost slots. */
+int flare_domain_forward_pack(flare_ctx* ctx, int phase, double* msg_lo, double* msg_hi);
+int flare_domain_forward_unpack(flare_ctx* ctx, int phase, const double* msg_lo_in, const double* msg_hi_in);
+
+/* Copy the rebuild signal (0 / non-zero) of the last evaluation to a DEVICE int32: all-reduce it (MAX) over the ranks
+   and rebuild when it is set.  Raised when an atom has moved trigger_displacement since the last rebuild. */
+int flare_domain_signal(flare_ctx* ctx, int32_t* flag_out);
+
+/* Global ids of the local atoms (owned first) -> DEVICE int64 [n_atoms]. */
+int flare_domain_get_tags(flare_ctx* ctx, int64_t* tags_out);
 
 /* Copy the state out; any pointer may be NULL.  Device-pointer version is asynchronous. */
 int flare_get_state(flare_ctx* ctx, double* pos, double* vel, double* e, double* f, double* var);

@@ -62,7 +62,15 @@ struct flare_ctx {
     int timing = 0;
     int sparse = 0;
     // binding
-    int64_t n = -1;
+    int64_t n = -1;      // atoms the kernels work on
+    int64_t n_cap = -1;  // atoms the workspace was carved for (n <= n_cap; they differ only in domain mode)
+    // domain decomposition (flare_domain_*): host mirrors of the device counters after flare_domain_commit
+    bool dom_active = false;
+    double dom_trigger = 0.0;       // displacement since the last rebuild that raises the rebuild signal
+    double dom_shift[4][3]{};       // frame shift of the send lists x-lo, x-hi, y-lo, y-hi
+    int dom_send[4]{}, dom_recv_cnt[4]{}, dom_recv_off[4]{};
+    int64_t dom_n_owned = 0;
+    int dom_list_cap = 0;
     Workspace ws{};
     cudaStream_t stream = nullptr;
     int chunk_cap = 0;
@@ -341,6 +349,9 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.scal = cv.take<double>(16);
     w.ascal = cv.take<unsigned long long>(18);
     w.qf_counter = cv.take<int>(kMaxGroups);
+    w.tag = cv.take<long long>(N);
+    w.dom = cv.take<int>(kDomInts);
+    w.send_idx = cv.take<int>(4 * (N / 2 + 1024));
     if (ws) *ws = w;
     if (chunk_out) *chunk_out = chunk;
     if (cells_out) *cells_out = (int)std::min<size_t>(cells, 0x7fffffff);
@@ -403,7 +414,7 @@ int evaluate(flare_ctx* c, Launcher& L, const double* pos, const int* types, dou
     {
         PhaseScope ps(c, FLARE_PHASE_NEIGHBOR);
         build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups, eff_skin(c),
-                        c->list_valid);
+                        c->list_valid, c->dom_active ? c->dom_trigger : 0.0);
         if (eff_skin(c) > 0.0) c->list_valid = true;
     }
     for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
@@ -599,7 +610,9 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     FLARE_CUDA(c, cudaSetDevice(c->device));
     carve(c, n_atoms, static_cast<char*>(workspace), &c->ws, &c->chunk_cap, &c->n_cells_cap);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->n = n_atoms;
+    c->n = c->n_cap = n_atoms;
+    c->dom_active = false;
+    c->dom_list_cap = (int)(std::max<int64_t>(n_atoms, 1) / 2 + 1024);
     c->state_set = c->forces_valid = c->var_valid = false;
     c->have_grid = false;
     c->pairf_valid = false;
@@ -608,6 +621,7 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.flags, 0, sizeof(int) * 4, c->stream));
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.scal, 0, sizeof(double) * 16, c->stream));  // thermostat xi = eta = 0
     if (c->ws.skin_gate) FLARE_CUDA(c, cudaMemsetAsync(c->ws.skin_gate, 0, sizeof(int) * 4, c->stream));
+    FLARE_CUDA(c, cudaMemsetAsync(c->ws.dom, 0, sizeof(int) * kDomInts, c->stream));
     return FLARE_OK;
 }
 
@@ -637,6 +651,8 @@ int flare_check(flare_ctx* c) {
         c->pairf_valid = false;
         c->forces_valid = c->var_valid = false;
     }
+    if (flags[0] & kFlagDomainOverflow)
+        return fail(c, FLARE_ERR_WORKSPACE_TOO_SMALL, "domain decomposition: a message buffer, a send list or the bound capacity is too small (or a peer sent a message of another step)");
     if (flags[0] & kFlagBadType) return fail(c, FLARE_ERR_INVALID_ARG, "a species index is outside 0..S-1");
     if (flags[0] & kFlagNonFinite) return fail(c, FLARE_ERR_NONFINITE, "non-finite position");
     if (flags[0] & kFlagNeighborOverflow)
@@ -848,6 +864,213 @@ int flare_step_nvt(flare_ctx* c, double dt_fs, int n_steps, int want_variance, d
         return fail(c, FLARE_ERR_INVALID_ARG, "thermostat temperature and time constant must be > 0");
     if (c->n >= 0 && c->n < 2) return fail(c, FLARE_ERR_INVALID_ARG, "the thermostat needs at least 2 atoms (g = 3N - 3)");
     return step_impl(c, dt_fs, n_steps, want_variance, T_kelvin, tau_fs);
+}
+
+// ---------------------------------------------------------------- multi-GPU domain decomposition (domain.cu)
+static int need_domain(flare_ctx* c) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!c->dom_active) return fail(c, FLARE_ERR_NOT_BOUND, "flare_domain_begin has not been called");
+    return FLARE_OK;
+}
+
+int flare_domain_begin(flare_ctx* c, int64_t n_owned, const double* pos, const double* vel, const int32_t* types,
+                       const int64_t* tags, const double box[9], const int pbc[3], double trigger_displacement) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (n_owned < 0 || n_owned > c->n_cap) return fail(c, FLARE_ERR_WORKSPACE_TOO_SMALL, "n_owned exceeds the bound capacity");
+    if (n_owned > 0 && (!pos || !types || !tags)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types/tags is null");
+    if (!(trigger_displacement >= 0.0)) return fail(c, FLARE_ERR_INVALID_ARG, "trigger displacement must be >= 0");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    c->n = n_owned;
+    rc = setup_grid(c, box, pbc);
+    if (rc) return rc;
+    const size_t n = (size_t)n_owned;
+    if (n > 0) {
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.x, pos, sizeof(double) * 3 * n, cudaMemcpyDeviceToDevice, c->stream));
+        if (vel) FLARE_CUDA(c, cudaMemcpyAsync(c->ws.v, vel, sizeof(double) * 3 * n, cudaMemcpyDeviceToDevice, c->stream));
+        else FLARE_CUDA(c, cudaMemsetAsync(c->ws.v, 0, sizeof(double) * 3 * n, c->stream));
+        FLARE_CUDA(c, cudaMemsetAsync(c->ws.f, 0, sizeof(double) * 3 * n, c->stream));
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.types, types, sizeof(int) * n, cudaMemcpyDeviceToDevice, c->stream));
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.tag, tags, sizeof(long long) * n, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    int h[kDomInts] = {0};
+    h[kDomNLocal] = h[kDomNOwned] = (int)n_owned;
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    FLARE_CUDA(c, cudaMemcpy(c->ws.dom, h, sizeof(h), cudaMemcpyHostToDevice));
+    c->dom_active = true;
+    c->dom_trigger = trigger_displacement;
+    c->dom_n_owned = n_owned;
+    for (int q = 0; q < 4; q++) c->dom_send[q] = c->dom_recv_cnt[q] = c->dom_recv_off[q] = 0;
+    c->state_set = true;
+    c->forces_valid = c->var_valid = false;
+    c->list_valid = false;
+    c->pairf_valid = false;
+    drop_step_graph(c);
+    return FLARE_OK;
+}
+
+int flare_domain_migrate_pack(flare_ctx* c, int axis, double lo_bound, double hi_bound, double shift_lo,
+                              double shift_hi, double* msg_lo, double* msg_hi, int64_t cap_rows) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (axis < 0 || axis > 2 || !msg_lo || !msg_hi || cap_rows < 0 || cap_rows > 0x7fffffff / kDomFullRow)
+        return fail(c, FLARE_ERR_INVALID_ARG, "bad axis, message pointer or capacity");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    const int nb = (int)c->n_cap;
+    dom_set_counts(L, c->ws, kDomNOwned, true, false);  // ghosts are dropped: the local set is the owned set
+    const double inf = HUGE_VAL;
+    const DomSel s{axis, kDomNOwned, -inf, lo_bound, hi_bound, inf};
+    int* leave_lo = c->ws.rank_in_cell;                // scratch (free between evaluations)
+    int* leave_hi = c->ws.rank_in_cell + (nb + 1) / 2;
+    int* stay = c->ws.cell_of;
+    dom_select(L, c->ws, s, nb, leave_lo, leave_hi, stay, std::max(nb / 2, 1));
+    dom_commit_lists(L, c->ws, kDomMig, kDomMig + 1, std::max(nb / 2, 1));
+    double sh[3] = {0.0, 0.0, 0.0};
+    sh[axis] = shift_lo;
+    dom_pack_full(L, c->ws, leave_lo, kDomMig, sh, true, msg_lo, (int)cap_rows);
+    sh[axis] = shift_hi;
+    dom_pack_full(L, c->ws, leave_hi, kDomMig + 1, sh, true, msg_hi, (int)cap_rows);
+    dom_compact_stay(L, c->ws, stay, nb);
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    c->list_valid = false;
+    c->pairf_valid = false;
+    return FLARE_OK;
+}
+
+int flare_domain_migrate_unpack(flare_ctx* c, const double* msg_lo_in, const double* msg_hi_in, int64_t cap_rows) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    if (msg_lo_in) dom_append(L, c->ws, msg_lo_in, (int)c->n_cap, (int)cap_rows, -1, true);
+    if (msg_hi_in) dom_append(L, c->ws, msg_hi_in, (int)c->n_cap, (int)cap_rows, -1, true);
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    return FLARE_OK;
+}
+
+int flare_domain_border_pack(flare_ctx* c, int phase, int axis, double lo_a, double lo_b, double hi_a, double hi_b,
+                             double shift_lo, double shift_hi, double* msg_lo, double* msg_hi, int64_t cap_rows) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (phase < 0 || phase > 1 || axis < 0 || axis > 2 || !msg_lo || !msg_hi || cap_rows < 0 ||
+        cap_rows > 0x7fffffff / kDomFullRow)
+        return fail(c, FLARE_ERR_INVALID_ARG, "bad phase, axis, message pointer or capacity");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    if (phase == 0) dom_set_counts(L, c->ws, kDomNOwned, true, false);  // a new ghost shell starts after the owned atoms
+    const DomSel s{axis, kDomNLocal, lo_a, lo_b, hi_a, hi_b};
+    int* list_lo = c->ws.send_idx + (size_t)(2 * phase) * c->dom_list_cap;
+    int* list_hi = c->ws.send_idx + (size_t)(2 * phase + 1) * c->dom_list_cap;
+    dom_select(L, c->ws, s, (int)c->n_cap, list_lo, list_hi, nullptr, c->dom_list_cap);
+    dom_commit_lists(L, c->ws, kDomSend + 2 * phase, kDomSend + 2 * phase + 1, c->dom_list_cap);
+    for (int side = 0; side < 2; side++) {
+        double* sh = c->dom_shift[2 * phase + side];
+        sh[0] = sh[1] = sh[2] = 0.0;
+        sh[axis] = side == 0 ? shift_lo : shift_hi;
+        dom_pack_full(L, c->ws, side == 0 ? list_lo : list_hi, kDomSend + 2 * phase + side, sh, c->forces_valid,
+                      side == 0 ? msg_lo : msg_hi, (int)cap_rows);
+    }
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    return FLARE_OK;
+}
+
+int flare_domain_border_unpack(flare_ctx* c, int phase, const double* msg_lo_in, const double* msg_hi_in,
+                               int64_t cap_rows) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (phase < 0 || phase > 1) return fail(c, FLARE_ERR_INVALID_ARG, "bad phase");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    // an absent neighbour (null) still records an empty ghost block
+    double* d_empty = c->ws.red;  // 8 doubles of reduction scratch
+    if (!msg_lo_in || !msg_hi_in) FLARE_CUDA(c, cudaMemsetAsync(d_empty, 0, sizeof(double) * kDomHeader, c->stream));
+    dom_append(L, c->ws, msg_lo_in ? msg_lo_in : d_empty, (int)c->n_cap, (int)cap_rows, 2 * phase, false);
+    dom_append(L, c->ws, msg_hi_in ? msg_hi_in : d_empty, (int)c->n_cap, (int)cap_rows, 2 * phase + 1, false);
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    return FLARE_OK;
+}
+
+int flare_domain_commit(flare_ctx* c, int64_t counts[14]) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    FLARE_CUDA(c, cudaStreamSynchronize(c->stream));
+    int h[kDomInts];
+    FLARE_CUDA(c, cudaMemcpy(h, c->ws.dom, sizeof(h), cudaMemcpyDeviceToHost));
+    rc = flare_check(c);  // message / list / capacity overflow of the rebuild
+    if (rc) return rc;
+    c->n = h[kDomNLocal];
+    c->dom_n_owned = h[kDomNOwned];
+    for (int q = 0; q < 4; q++) {
+        c->dom_send[q] = h[kDomSend + q];
+        c->dom_recv_cnt[q] = h[kDomRecvCnt + q];
+        c->dom_recv_off[q] = h[kDomRecvOff + q];
+    }
+    FLARE_CUDA(c, cudaMemsetAsync(c->ws.dom + kDomNeed, 0, sizeof(int), c->stream));
+    c->list_valid = false;  // membership changed: the candidate list is rebuilt by the next evaluation
+    c->pairf_valid = false;
+    drop_step_graph(c);
+    if (counts) {
+        counts[0] = h[kDomNLocal];
+        counts[1] = h[kDomNOwned];
+        for (int q = 0; q < 4; q++) {
+            counts[2 + q] = h[kDomSend + q];
+            counts[6 + q] = h[kDomRecvCnt + q];
+            counts[10 + q] = h[kDomRecvOff + q];
+        }
+    }
+    return FLARE_OK;
+}
+
+int flare_domain_forward_pack(flare_ctx* c, int phase, double* msg_lo, double* msg_hi) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (phase < 0 || phase > 1 || !msg_lo || !msg_hi) return fail(c, FLARE_ERR_INVALID_ARG, "bad phase or message pointer");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    for (int side = 0; side < 2; side++) {
+        const int q = 2 * phase + side;
+        dom_pack_fwd(L, c->ws, c->ws.send_idx + (size_t)q * c->dom_list_cap, c->dom_send[q], c->dom_shift[q],
+                     side == 0 ? msg_lo : msg_hi);
+    }
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    return FLARE_OK;
+}
+
+int flare_domain_forward_unpack(flare_ctx* c, int phase, const double* msg_lo_in, const double* msg_hi_in) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (phase < 0 || phase > 1) return fail(c, FLARE_ERR_INVALID_ARG, "bad phase");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    if (msg_lo_in) dom_unpack_fwd(L, c->ws, msg_lo_in, c->dom_recv_off[2 * phase], c->dom_recv_cnt[2 * phase]);
+    if (msg_hi_in) dom_unpack_fwd(L, c->ws, msg_hi_in, c->dom_recv_off[2 * phase + 1], c->dom_recv_cnt[2 * phase + 1]);
+    if (L.err != cudaSuccess) return cuda_fail(c, L.err, L.err_where ? L.err_where : "domain launch");
+    return FLARE_OK;
+}
+
+int flare_domain_signal(flare_ctx* c, int32_t* flag_out) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (!flag_out) return fail(c, FLARE_ERR_INVALID_ARG, "flag pointer is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    if (eff_skin(c) > 0.0 && c->dom_trigger > 0.0)
+        FLARE_CUDA(c, cudaMemcpyAsync(flag_out, c->ws.dom + kDomNeed, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
+    else
+        FLARE_CUDA(c, cudaMemsetAsync(flag_out, 1, 1, c->stream));  // no candidate list, no displacement tracking: always
+    return FLARE_OK;
+}
+
+int flare_domain_get_tags(flare_ctx* c, int64_t* tags_out) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (!tags_out && c->n > 0) return fail(c, FLARE_ERR_INVALID_ARG, "tags pointer is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    if (c->n > 0)
+        FLARE_CUDA(c, cudaMemcpyAsync(tags_out, c->ws.tag, sizeof(long long) * (size_t)c->n, cudaMemcpyDeviceToDevice, c->stream));
+    return FLARE_OK;
 }
 
 int flare_get_thermostat(flare_ctx* c, double* xi, double* eta) {

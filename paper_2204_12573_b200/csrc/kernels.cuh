@@ -13,6 +13,26 @@ constexpr int kMaxGroups = 64;  // quadratic-form groups: (central species) or (
 constexpr int kNumPhases = 6;
 constexpr int kSkinStride = 64;  // row stride of the skin (candidate) list: one 64-bit hit mask per atom
 
+// ---- domain decomposition (domain.cu): device-side counters Workspace::dom[] and message layout
+constexpr int kDomNLocal = 0;   // atoms in the state arrays: owned + ghosts appended so far
+constexpr int kDomNOwned = 1;   // owned atoms (the first ones)
+constexpr int kDomSend = 2;     // [4] entries of the send lists x-lo, x-hi, y-lo, y-hi
+constexpr int kDomRecvCnt = 6;  // [4] ghosts received from x-lo, x-hi, y-lo, y-hi
+constexpr int kDomRecvOff = 10; // [4] first slot of each of those ghost blocks
+constexpr int kDomNeed = 15;    // non-zero: an atom has moved further than the halo skin allows since the last rebuild
+constexpr int kDomTot = 16;     // [3] totals of the running selection (lo, hi, stay)
+constexpr int kDomMig = 20;     // [2] atoms leaving through the lo / hi face of the running migration phase
+constexpr int kDomInts = 32;
+constexpr int kDomHeader = 8;   // doubles before the first row of a message ([0] = row count)
+constexpr int kDomFullRow = 11; // x, v, f, type, tag
+constexpr int kDomFwdRow = 9;   // x, v, f
+
+// selection along one axis: bit 0 = coordinate in [lo_a, lo_b), bit 1 = in [hi_a, hi_b); over the first dom[n_from] atoms
+struct DomSel {
+    int axis, n_from;
+    double lo_a, lo_b, hi_a, hi_b;
+};
+
 // Per-context launch state: the dynamic shared-memory limit a kernel has been configured for and its occupancy.
 // cudaFuncSetAttribute acts on the CURRENT device only, so this lives in the context (one context = one device),
 // not in function-local statics: a second context on another GPU of the same process configures its own copy.
@@ -177,6 +197,10 @@ struct Workspace {
     double* scal = nullptr;                // [16]: [0..8] virial, [12..15] thermostat xi, eta, scale, K2
     unsigned long long* ascal = nullptr;   // [18] analysis outputs (max bits, count, coordination histogram)
     int* qf_counter = nullptr;             // [kMaxGroups] tile queues of the quadratic-form launches
+    // ---- domain decomposition
+    long long* tag = nullptr;  // [N] global atom id (travels with the atom)
+    int* dom = nullptr;        // [kDomInts] counters, see kDom*
+    int* send_idx = nullptr;   // [4][N/2 + 1024] send lists of the two exchange phases
 };
 constexpr int kRedBlocksMax = 1184;
 
@@ -225,7 +249,8 @@ struct GroupDev {
 // skin > 0: keep a candidate list with cutoffs r_cut + skin across evaluations (list_valid: one exists for this
 // order / box / types) and filter it with the exact predicate; skin = 0: rebuild everything every time.
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
-                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid);
+                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid,
+                     double dom_trigger = 0.0);  // > 0: raise Workspace::dom[kDomNeed] once an atom has moved that far
 
 // Descriptor rows [row0,row0+nrows): compact A -> ws.A, UNNORMALISED B -> bh_out (row r at (r - row0)*ld),
 // ||B|| -> nrm_out.  One launch per group.
@@ -253,5 +278,17 @@ void run_analyze(Launcher& L, const Grid& g, const Workspace& ws, int n, int mma
                  unsigned long long* out18);
 void run_nh_half(Launcher& L, const Workspace& ws, int n, const double* mass_dev, double h, double gkT, double Q,
                  double* thermo);
+
+// domain.cu: selection / packing / compaction kernels of the domain decomposition (all sizes on the device)
+void dom_select(Launcher& L, const Workspace& ws, const DomSel& s, int n_bound, int* list_lo, int* list_hi,
+                int* list_stay, int cap);
+void dom_commit_lists(Launcher& L, const Workspace& ws, int slot_lo, int slot_hi, int cap);
+void dom_pack_full(Launcher& L, const Workspace& ws, const int* list, int cnt_slot, const double shift[3],
+                   bool with_force, double* msg, int cap_rows);
+void dom_append(Launcher& L, const Workspace& ws, const double* msg, int n_cap, int max_rows, int slot, bool owned);
+void dom_compact_stay(Launcher& L, const Workspace& ws, const int* list_stay, int n_bound);
+void dom_set_counts(Launcher& L, const Workspace& ws, int from_slot, bool to_local, bool to_owned);
+void dom_pack_fwd(Launcher& L, const Workspace& ws, const int* list, int cnt, const double shift[3], double* msg);
+void dom_unpack_fwd(Launcher& L, const Workspace& ws, const double* msg, int off, int cnt);
 
 }  // namespace flare

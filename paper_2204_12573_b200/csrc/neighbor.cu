@@ -446,9 +446,14 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
 // rebuilds.  The threshold is taken a hair low so that the triangle inequality holds with rounding to spare.
 // In a captured step (CUDA graph, small systems) the decision also drives the IF node that holds the rebuild chain.
 __global__ void k_gate_decide(Basis bs, double reach, const int* __restrict__ dmax, int* __restrict__ gate,
-                              cudaGraphConditionalHandle cond, int use_cond) {
+                              cudaGraphConditionalHandle cond, int use_cond, float dom_trigger, int* __restrict__ dom_need) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     int need = *gate;  // k_refresh raises it for a non-finite position or a changed species
+    if (dom_need) {  // domain decomposition: the ghost shell has dom_trigger of slack per atom (domain.cu)
+        float m = 0.f;
+        for (int a = 0; a < bs.S; a++) m = fmaxf(m, __int_as_float(dmax[a]));
+        if (m >= dom_trigger || need) *dom_need = 1;
+    }
     for (int a = 0; a < bs.S; a++)
         for (int b = a; b < bs.S; b++) {
             const double da = __int_as_float(dmax[a]), db = __int_as_float(dmax[b]);
@@ -648,7 +653,8 @@ k_group_assign(int n, int S, int sparse, int n_groups, const AtomS* __restrict__
 
 // ------------------------------------------------------------------ host-side driver of a1
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
-                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid) {
+                     const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid,
+                     double dom_trigger) {
     if (n == 0) return;
     const int tb = 256;
     const bool use_skin = skin > 0.0;
@@ -676,7 +682,7 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
             const bool as_if = L.capturing;
             const cudaGraphConditionalHandle h = as_if ? L.cond_handle() : 0;
             L.launch(k_gate_decide, dim3(1), dim3(32), 0, bs, reach, (const int*)(ws.skin_gate + 4), ws.skin_gate, h,
-                     as_if ? 1 : 0);
+                     as_if ? 1 : 0, (float)dom_trigger, dom_trigger > 0.0 ? ws.dom + kDomNeed : (int*)nullptr);
             if (as_if) { L.begin_if(h); gate = nullptr; }
         }
     }

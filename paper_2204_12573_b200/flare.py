@@ -33,7 +33,11 @@ EXPORTS = (
     "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_rows", "flare_get_timings", "flare_kernel_launches",
     "flare_last_error",
     "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_analyze",
+    "flare_domain_begin", "flare_domain_migrate_pack", "flare_domain_migrate_unpack", "flare_domain_border_pack",
+    "flare_domain_border_unpack", "flare_domain_commit", "flare_domain_forward_pack", "flare_domain_forward_unpack",
+    "flare_domain_signal", "flare_domain_get_tags",
 )
+MSG_HEADER, MSG_FULL_ROW, MSG_FWD_ROW = 8, 11, 9  # message layout of the domain data plane (doubles)
 
 
 class FlareError(RuntimeError):
@@ -88,6 +92,16 @@ def load_library():
     lib.flare_set_thermostat.argtypes = [vp, dbl, dbl]
     lib.flare_get_virial.argtypes = [vp, vp]
     lib.flare_analyze.argtypes = [vp, dbl, i32, i32, dbl, C.POINTER(dbl), C.POINTER(i64), vp, vp]
+    lib.flare_domain_begin.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, dbl]
+    lib.flare_domain_migrate_pack.argtypes = [vp, i32, dbl, dbl, dbl, dbl, vp, vp, i64]
+    lib.flare_domain_migrate_unpack.argtypes = [vp, vp, vp, i64]
+    lib.flare_domain_border_pack.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, vp, vp, i64]
+    lib.flare_domain_border_unpack.argtypes = [vp, i32, vp, vp, i64]
+    lib.flare_domain_commit.argtypes = [vp, vp]
+    lib.flare_domain_forward_pack.argtypes = [vp, i32, vp, vp]
+    lib.flare_domain_forward_unpack.argtypes = [vp, i32, vp, vp]
+    lib.flare_domain_signal.argtypes = [vp, vp]
+    lib.flare_domain_get_tags.argtypes = [vp, vp]
     _lib = lib
     return lib
 
@@ -300,13 +314,14 @@ class Flare:
         return dict(max_unc=mx.value if uncertainty else None, n_above=na.value if uncertainty else None,
                     coord=coord, hist=hist if coordination else None)
 
-    def get_state(self, variances: bool = False):
-        """Device tensors dict(pos, vel, E, F[, V])."""
+    def get_state(self, variances: bool = False, results: bool = True):
+        """Device tensors dict(pos, vel, E, F[, V]); results=False: positions and velocities only (no evaluation needed)."""
         torch = self._torch
         n = self.n_atoms
         mk = lambda *s: torch.empty(s, dtype=torch.float64, device=self.device)
-        pos, vel, e, f = mk(n, 3), mk(n, 3), mk(n), mk(n, 3)
-        v = mk(n) if variances else None
+        pos, vel = mk(n, 3), mk(n, 3)
+        e, f = (mk(n), mk(n, 3)) if results else (None, None)
+        v = mk(n) if (variances and results) else None
         ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
         self._check(self._lib.flare_get_state(self._ctx, ptr(pos), ptr(vel), ptr(e), ptr(f), ptr(v)))
         self.check()
@@ -320,6 +335,57 @@ class Flare:
         self._check(self._lib.flare_get_state_host(self._ctx, _hp(out["pos"]), _hp(out["vel"]), _hp(out["E"]),
                                                    _hp(out["F"]), _hp(out.get("V"))))
         return out
+
+    # ------------------------------------------------------------------ domain decomposition (device data plane)
+    def _msg(self, t):
+        return None if t is None else self._dev(t, self._torch.float64, tuple(t.shape))
+
+    def domain_begin(self, n_owned, pos, vel, types, tags, box, pbc, trigger: float):
+        torch = self._torch
+        n = int(n_owned)
+        boxh, pbch = _box9(box), _np(pbc, np.int32)
+        self._check(self._lib.flare_domain_begin(
+            self._ctx, n, self._dev(pos, torch.float64, (n, 3)), None if vel is None else self._dev(vel, torch.float64, (n, 3)),
+            self._dev(types, torch.int32, (n,)), self._dev(tags, torch.int64, (n,)), _hp(boxh), _hp(pbch), float(trigger)))
+        self.n_atoms = n
+
+    def domain_migrate_pack(self, axis, lo_bound, hi_bound, shift_lo, shift_hi, msg_lo, msg_hi, cap_rows):
+        self._check(self._lib.flare_domain_migrate_pack(self._ctx, int(axis), float(lo_bound), float(hi_bound), float(shift_lo),
+                                                        float(shift_hi), self._msg(msg_lo), self._msg(msg_hi), int(cap_rows)))
+
+    def domain_migrate_unpack(self, msg_lo_in, msg_hi_in, cap_rows):
+        self._check(self._lib.flare_domain_migrate_unpack(self._ctx, self._msg(msg_lo_in), self._msg(msg_hi_in), int(cap_rows)))
+
+    def domain_border_pack(self, phase, axis, lo_a, lo_b, hi_a, hi_b, shift_lo, shift_hi, msg_lo, msg_hi, cap_rows):
+        self._check(self._lib.flare_domain_border_pack(self._ctx, int(phase), int(axis), float(lo_a), float(lo_b), float(hi_a),
+                                                       float(hi_b), float(shift_lo), float(shift_hi), self._msg(msg_lo),
+                                                       self._msg(msg_hi), int(cap_rows)))
+
+    def domain_border_unpack(self, phase, msg_lo_in, msg_hi_in, cap_rows):
+        self._check(self._lib.flare_domain_border_unpack(self._ctx, int(phase), self._msg(msg_lo_in), self._msg(msg_hi_in),
+                                                         int(cap_rows)))
+
+    def domain_commit(self):
+        """-> dict(n_local, n_owned, send[4], recv[4], recv_off[4]); n_atoms becomes n_local."""
+        c = np.zeros(14, np.int64)
+        self._check(self._lib.flare_domain_commit(self._ctx, _hp(c)))
+        self.n_atoms = int(c[0])
+        return dict(n_local=int(c[0]), n_owned=int(c[1]), send=[int(v) for v in c[2:6]], recv=[int(v) for v in c[6:10]],
+                    recv_off=[int(v) for v in c[10:14]])
+
+    def domain_forward_pack(self, phase, msg_lo, msg_hi):
+        self._check(self._lib.flare_domain_forward_pack(self._ctx, int(phase), self._msg(msg_lo), self._msg(msg_hi)))
+
+    def domain_forward_unpack(self, phase, msg_lo_in, msg_hi_in):
+        self._check(self._lib.flare_domain_forward_unpack(self._ctx, int(phase), self._msg(msg_lo_in), self._msg(msg_hi_in)))
+
+    def domain_signal(self, flag):
+        self._check(self._lib.flare_domain_signal(self._ctx, self._dev(flag, self._torch.int32, (1,))))
+
+    def domain_tags(self):
+        t = self._torch.empty(self.n_atoms, dtype=self._torch.int64, device=self.device)
+        self._check(self._lib.flare_domain_get_tags(self._ctx, C.c_void_p(t.data_ptr())))
+        return t
 
     # ------------------------------------------------------------------ hooks
     def neighbors(self, stride: int | None = None):

@@ -1,281 +1,323 @@
-"""Multi-GPU path: spatial domain decomposition with one halo exchange per
-evaluation -- what the paper gets from LAMMPS ("All ... GPU-GPU communication is handled by LAMMPS";
-weak scaling P:L239).  One process per GPU; `torch.distributed` point-to-point messages between neighbouring
-slabs (NCCL over NVLink on GPUs, gloo in the CPU tests).  Everything the force field computes still runs in
-the CUDA kernels behind the C ABI: this module only decides which atoms go where (argument marshalling).
+"""Multi-GPU path: spatial domain decomposition on a 2-D (x, y) process grid with one
+halo exchange per MD step -- what the paper gets from LAMMPS ("MD runs entirely on GPUs with zero CPU-GPU
+data transfer except for I/O ... GPU-GPU communication"; weak scaling P:L239; "near-two-dimensional" P:L233).
 
-Decomposition: the box is cut along one periodic axis into `world` slabs of width w = L / world; rank r owns
-the atoms with coordinate in [r w, (r+1) w).  Each rank evaluates its owned atoms together with GHOST copies
-of every atom within g = 2 max r_cut of its slab: with a halo two cutoffs wide the local energies of the ghosts
-that neighbour an owned atom are themselves complete, so the forces on owned atoms,
-F_k = sum_j (dE_k/dr_kj - dE_j/dr_jk), need no reverse (force) exchange and the gather stays atomics-free.
-Inside a rank the slab is an OPEN dimension of length w + 2 g (local coordinate = offset from the slab centre,
-nearest image); the other two dimensions keep their boundary conditions.
+One process per GPU.  This module is the HOST ORCHESTRATION only: it knows the geometry of the process grid (a few
+scalars), decides which message goes to which rank, and moves message buffers with `torch.distributed`
+point-to-point calls (NCCL over NVLink on GPUs; gloo in the CPU tests).  It does no arithmetic on atom data: selecting
+the atoms of a face, packing and shifting them, compacting, appending ghosts, the per-step gather / scatter of
+(x, v, F) and the rebuild decision all run in the library's CUDA kernels behind the C ABI (`flare_domain_*`,
+csrc/domain.cu), with every count kept on the device.
 
-Per MD step: (1) halo exchange of (x, v, F, type) of the atoms near the two faces -- ghosts carry their owner's
-velocity and force so that the library's integrator moves them exactly as their owner does; (2) one
-`Engine.md_step` on owned + ghosts; (3) migration of owned atoms that left the slab (with v, F, global id).
-Requirements: w >= g (only adjacent slabs talk), w >= 2 g when world == 2 (no atom is a ghost twice), and
-atoms move less than w per step.
+Geometry.  The box is cut into px x py rectangles of widths w = L / p along the decomposed axes.  A rank evaluates
+its owned atoms together with GHOST copies of every atom within the halo width h = 2 max r_cut + halo_skin of its
+rectangle: with a halo two cutoffs wide the local energies of the ghosts that neighbour an owned atom are complete, so
+F_k = sum_j (dE_k/dr_kj - dE_j/dr_jk) of an owned atom needs no reverse (force) exchange and the gather stays
+atomics-free.  Local frame: a decomposed dimension is open, of length w + 2 h, with the owned rectangle at
+[h, h + w); the frame of the lo (hi) neighbour is shifted by +w (-w), so periodic images need no special case.
+Ghosts are exchanged in two phases (x, then y including the x ghosts: corners).
+
+Time line.  REBUILD (all ranks together): migrate owned atoms that left the rectangle, select the atoms of the
+four face strips (fixed send lists), exchange full rows at fixed message capacity with the count in the header (no
+size round trip), append the ghosts after the owned atoms, one synchronisation to learn the new local count.
+STEP (between rebuilds; nothing blocks the host): forward rows (x, v, F) of the fixed lists -> fixed ghost slots,
+`flare_step(dt, 1)` on owned + ghosts (ghosts carry their owner's velocity and force, so the integrator moves them as
+their owner does), rebuild signal.  Membership, order and counts are stable between rebuilds, so the context's
+candidate neighbour list survives.  The signal -- "some atom has moved `trigger` since the rebuild", raised on the
+device by the same kernel that gates the candidate list -- is all-reduced (MAX) asynchronously and read `lag` steps
+later, so every rank takes the same decision without a per-step host synchronisation; the halo skin covers
+2 x trigger plus the motion of those `lag` steps (trigger = 0.35 halo_skin).
 """
 from __future__ import annotations
+
+import collections
 
 import numpy as np
 import torch
 import torch.distributed as dist
 
+MSG_HEADER, MSG_FULL_ROW, MSG_FWD_ROW = 8, 11, 9  # include/flare_b200.h: message layout (doubles)
+
 
 class Engine:
-    """What the decomposition needs from a force engine.  Tensors live on `device`."""
+    """What the decomposition needs from a force engine: the device data plane of include/flare_b200.h."""
 
     device = torch.device("cpu")
 
-    def evaluate(self, pos, types, box, pbc, variances):  # -> E [n], F [n,3], V [n] or None
-        raise NotImplementedError
-
-    def md_step(self, pos, vel, frc, types, box, pbc, dt, variances):  # -> pos, vel, E, F, V
-        raise NotImplementedError
+    def begin(self, pos, vel, types, tags, box, pbc, trigger): raise NotImplementedError
+    def migrate_pack(self, axis, lo_bound, hi_bound, shift_lo, shift_hi, msg_lo, msg_hi, cap): raise NotImplementedError
+    def migrate_unpack(self, msg_lo_in, msg_hi_in, cap): raise NotImplementedError
+    def border_pack(self, phase, axis, lo_a, lo_b, hi_a, hi_b, shift_lo, shift_hi, msg_lo, msg_hi, cap): raise NotImplementedError
+    def border_unpack(self, phase, msg_lo_in, msg_hi_in, cap): raise NotImplementedError
+    def commit(self): raise NotImplementedError            # -> dict(n_local, n_owned, send[4], recv[4], recv_off[4])
+    def forward_pack(self, phase, msg_lo, msg_hi): raise NotImplementedError
+    def forward_unpack(self, phase, msg_lo_in, msg_hi_in): raise NotImplementedError
+    def step(self, dt, n_steps, variances): raise NotImplementedError   # n_steps = 0: forces of the current positions
+    def signal(self, flag): raise NotImplementedError      # flag: int32[1] tensor on `device`
+    def owned(self, variances): raise NotImplementedError  # -> host dict(tags, pos (local frame), vel, E, F, V)
 
 
 class CudaEngine(Engine):
-    """The product engine: libflare_b200 through its binding.  The workspace is sized once for `capacity` atoms."""
+    """The product engine: libflare_b200 through its binding.  The workspace is bound once, for `capacity` atoms."""
 
     def __init__(self, flare_ctx, capacity: int):
         self.ctx = flare_ctx
         self.device = flare_ctx.device
         self.capacity = int(capacity)
-        self._ws = None
+        self.ctx.bind(self.capacity)
+        self.skin = 1e-3 * self.ctx.get_option(5)  # FLARE_OPT_SKIN_MILLI_ANGSTROM
+        self.n_owned = 0
 
-    def _bind(self, n):
+    def begin(self, pos, vel, types, tags, box, pbc, trigger):
+        dev = self.device
+        n = len(tags)
         if n > self.capacity:
-            raise ValueError(f"{n} local atoms exceed the engine capacity {self.capacity}")
-        if self._ws is None:
-            self.ctx.bind(self.capacity)  # allocates the workspace for the capacity
-            self._ws = self.ctx._workspace
-        if self.ctx.n_atoms != n:  # re-binding drops the candidate neighbour list: only when the size changed
-            self.ctx.bind(n, workspace=self._ws)
+            raise ValueError(f"{n} owned atoms exceed the engine capacity {self.capacity}")
+        self.ctx.domain_begin(n, torch.as_tensor(pos, dtype=torch.float64).reshape(n, 3).to(dev),
+                              torch.as_tensor(vel, dtype=torch.float64).reshape(n, 3).to(dev),
+                              torch.as_tensor(types, dtype=torch.int32).to(dev), torch.as_tensor(tags, dtype=torch.int64).to(dev),
+                              box, pbc, trigger)
+        self.n_owned = n
 
-    def evaluate(self, pos, types, box, pbc, variances):
-        self._bind(pos.shape[0])
-        e, f, v = self.ctx.compute(pos.contiguous(), types.contiguous(), box, pbc, variances=variances)
-        return e, f, v
+    def migrate_pack(self, *a): self.ctx.domain_migrate_pack(*a)
+    def migrate_unpack(self, *a): self.ctx.domain_migrate_unpack(*a)
+    def border_pack(self, *a): self.ctx.domain_border_pack(*a)
+    def border_unpack(self, *a): self.ctx.domain_border_unpack(*a)
 
-    def md_step(self, pos, vel, frc, types, box, pbc, dt, variances):
-        self._bind(pos.shape[0])
-        self.ctx.set_state(pos.contiguous(), vel.contiguous(), types.contiguous(), box, pbc)
-        self.ctx.set_forces(frc.contiguous())
-        self.ctx.step(dt, 1, want_variance=variances)
+    def commit(self):
+        c = self.ctx.domain_commit()
+        self.n_owned = c["n_owned"]
+        return c
+
+    def forward_pack(self, *a): self.ctx.domain_forward_pack(*a)
+    def forward_unpack(self, *a): self.ctx.domain_forward_unpack(*a)
+
+    def step(self, dt, n_steps, variances):
+        self.ctx.step(dt, n_steps, want_variance=variances)
+
+    def signal(self, flag): self.ctx.domain_signal(flag)
+
+    def owned(self, variances):
+        n = self.n_owned
         st = self.ctx.get_state(variances=variances)
-        return st["pos"], st["vel"], st["E"], st["F"], st["V"]
+        out = {k: (st[k][:n].cpu().numpy() if st[k] is not None else None) for k in ("pos", "vel", "E", "F", "V")}
+        out["tags"] = self.ctx.domain_tags()[:n].cpu().numpy()
+        return out
 
 
-class SlabDecomposition:
-    """State of one rank: its owned atoms (global coordinates) and the geometry of its slab."""
+class DomainDecomposition:
+    """One rank of a px x py process grid over two axes of an orthorhombic box (rank = cx * py + cy)."""
 
-    def __init__(self, engine: Engine, box, pbc, r_cut_max: float, axis: int = 0, group=None):
+    def __init__(self, engine: Engine, box, pbc, r_cut_max: float, grid=None, axes=(0, 1), halo_skin: float = 1.2,
+                 lag: int = 2, border_capacity: int | None = None, migrate_capacity: int = 8192, self_halo: bool = False,
+                 group=None):
         self.engine = engine
         self.group = group
         self.world = dist.get_world_size(group) if dist.is_initialized() else 1
         self.rank = dist.get_rank(group) if dist.is_initialized() else 0
-        self.axis = int(axis)
+        if grid is None:
+            grid = (self.world, 1)
+        if grid[0] * grid[1] != self.world:
+            raise ValueError(f"process grid {grid} does not match the world size {self.world}")
         b = np.asarray(box, dtype=np.float64).reshape(-1)
         self.L = (np.diag(b.reshape(3, 3)) if b.size == 9 else b.reshape(3)).copy()
         self.pbc = np.asarray(pbc, dtype=np.int32).reshape(3).copy()
-        self.g = 2.0 * float(r_cut_max)
-        self.w = self.L[self.axis] / self.world
-        if self.world > 1:
-            if not self.pbc[self.axis]:
-                raise ValueError("the decomposed axis must be periodic")
-            if self.w < self.g or (self.world == 2 and self.w < 2.0 * self.g):
-                raise ValueError(f"slab width {self.w:.3f} too small for a halo of {self.g:.3f} on {self.world} ranks")
-        self.lo = self.rank * self.w
-        self.centre = self.lo + 0.5 * self.w
-        # local box: the slab plus its halo, open along the axis
+        self.h = 2.0 * float(r_cut_max) + float(halo_skin)
+        self.trigger = 0.35 * float(halo_skin)
+        # the engine's own candidate list may restart the displacement tracking when ITS skin is used up (that raises the
+        # signal too); until the rebuild `lag` steps later an atom may have moved that skin: it must fit into half the halo skin
+        if getattr(engine, "skin", 0.0) > 0.4 * float(halo_skin):
+            raise ValueError(f"halo_skin {halo_skin} must be at least 2.5 x the engine's list skin {engine.skin}")
+        self.lag = max(1, int(lag))
+        coords = (self.rank // grid[1], self.rank % grid[1])
+        # decomposed axes = exchange phases, in order
+        self.phases = []
         self.local_L = self.L.copy()
         self.local_pbc = self.pbc.copy()
-        if self.world > 1:
-            self.local_L[self.axis] = self.w + 2.0 * self.g
-            self.local_pbc[self.axis] = 0
+        self.lo = np.zeros(3)
+        for axis, p, c in zip(axes, grid, coords):
+            # an axis with one rank keeps its periodic boundary inside the engine -- unless self_halo asks for the
+            # full data path on it too (the rank is then its own neighbour on both sides: its ghosts are its own
+            # periodic images; used to exercise and time the data plane on one GPU)
+            if p == 1 and not (self_halo and self.pbc[axis]):
+                continue
+            if not self.pbc[axis]:
+                raise ValueError("a decomposed axis must be periodic")
+            w = self.L[axis] / p
+            if w < self.h:
+                raise ValueError(f"domain width {w:.3f} along axis {axis} is smaller than the halo {self.h:.3f}")
+            step = grid[1] if axis == axes[0] else 1
+            base = self.rank - c * step
+            self.phases.append(dict(axis=axis, p=p, c=c, w=w, lo_rank=base + ((c - 1) % p) * step,
+                                    hi_rank=base + ((c + 1) % p) * step))
+            self.local_L[axis] = w + 2.0 * self.h
+            self.local_pbc[axis] = 0
+            self.lo[axis] = c * w - self.h  # global coordinate of the local origin
         self.local_box = np.diag(self.local_L).reshape(9)
-        self.pos = self.vel = self.frc = self.types = self.gid = None
-        self.E = self.V = None
+        self.border_capacity = border_capacity
+        self.migrate_capacity = int(migrate_capacity)
+        self.counts = None
+        self.built = False
+        self.rebuilds = 0
         self.bytes_sent = 0
+        self._flags = collections.deque()
+        self._fwd = None
 
-    # ------------------------------------------------------------------ geometry
-    def owner_of(self, x_axis):
-        """Rank owning a (wrapped) coordinate along the axis."""
-        r = torch.floor(x_axis / self.w).to(torch.int64)
-        return torch.clamp(r, 0, self.world - 1)
-
-    def _wrap_axis(self, pos):
-        if self.world > 1 or self.pbc[self.axis]:
-            L = self.L[self.axis]
-            x = pos[:, self.axis]
-            x = x - L * torch.floor(x / L)
-            x = torch.where(x >= L, torch.zeros_like(x), x)
-            pos = pos.clone()
-            pos[:, self.axis] = x
-        return pos
-
-    def _to_local(self, pos):
-        """Global -> local coordinates (nearest image to the slab centre, shifted so that the slab starts at g)."""
-        if self.world == 1:
-            return pos
-        L = self.L[self.axis]
-        d = pos[:, self.axis] - self.centre
-        d = d - L * torch.round(d / L)
-        out = pos.clone()
-        out[:, self.axis] = d + 0.5 * self.w + self.g
-        return out
-
-    def _to_global(self, pos_local):
-        if self.world == 1:
-            return pos_local
-        out = pos_local.clone()
-        out[:, self.axis] = pos_local[:, self.axis] - self.g + self.lo
-        return self._wrap_axis(out)
-
-    # ------------------------------------------------------------------ scatter the initial system
+    # ------------------------------------------------------------------ initial distribution and collection (I/O)
     def scatter(self, pos, vel, types):
-        """Every rank passes the same full system (host arrays); each keeps the atoms of its slab."""
-        dev = self.engine.device
-        pos = torch.as_tensor(np.asarray(pos, dtype=np.float64).reshape(-1, 3))
-        pos = self._wrap_axis(pos)
-        mine = self.owner_of(pos[:, self.axis]) == self.rank if self.world > 1 else torch.ones(len(pos), dtype=torch.bool)
-        idx = torch.nonzero(mine).reshape(-1)
-        self.gid = idx.to(dev)
-        self.pos = pos[idx].to(dev)
-        v = np.zeros((len(pos), 3)) if vel is None else np.asarray(vel, dtype=np.float64).reshape(-1, 3)
-        self.vel = torch.as_tensor(v)[idx].to(dev)
-        self.types = torch.as_tensor(np.asarray(types, dtype=np.int32))[idx].to(dev)
-        self.frc = None
+        """Every rank passes the same full system (host arrays); each keeps the atoms of its rectangle, in its frame."""
+        pos = np.array(pos, dtype=np.float64).reshape(-1, 3)
+        n_all = len(pos)
+        vel = np.zeros((n_all, 3)) if vel is None else np.asarray(vel, dtype=np.float64).reshape(-1, 3)
+        types = np.asarray(types, dtype=np.int32).reshape(-1)
+        mine = np.ones(n_all, dtype=bool)
+        for ph in self.phases:
+            a, Lx = ph["axis"], self.L[ph["axis"]]
+            x = pos[:, a] - Lx * np.floor(pos[:, a] / Lx)
+            x[x >= Lx] = 0.0
+            pos[:, a] = x
+            mine &= np.clip(np.floor(x / ph["w"]).astype(np.int64), 0, ph["p"] - 1) == ph["c"]
+        idx = np.nonzero(mine)[0]
+        local = pos[idx] - self.lo[None, :]
+        if self.border_capacity is None and self.phases:
+            # the same on every rank (both ends of a message must agree on its size): a face strip of a rectangle of
+            # uniform density, widened by the ghosts of the first phase, with 50 % to spare
+            q = max(self.h / ph["w"] for ph in self.phases)
+            self.border_capacity = int(1.5 * (n_all / self.world) * q * (1.0 + 2.0 * q)) + 4096
+        self.engine.begin(local, vel[idx], types[idx], idx.astype(np.int64), self.local_box, self.local_pbc, self.trigger)
+        self.built = False
+        self._flags.clear()
         return self
 
-    # ------------------------------------------------------------------ messages
-    def _exchange(self, to_left, to_right):
-        """Send one payload [n, c] (float64) to each neighbour, receive theirs.  Returns (from_left, from_right)."""
-        left, right = (self.rank - 1) % self.world, (self.rank + 1) % self.world
-        host = dist.get_backend(self.group) == "gloo"
-        dev = self.engine.device
-        c = to_left.shape[1]
-        send = [t.cpu() if host else t.contiguous() for t in (to_left, to_right)]
-        cdev = torch.device("cpu") if host else dev
-        n_out = torch.tensor([send[0].shape[0], send[1].shape[0]], dtype=torch.int64, device=cdev)
-        n_in = torch.zeros(2, dtype=torch.int64, device=cdev)
-        # sizes first: my "to_left" count goes to the left neighbour, who stores it as its "from_right" count
-        ops = [dist.P2POp(dist.isend, n_out[0:1], left, self.group, tag=1), dist.P2POp(dist.isend, n_out[1:2], right, self.group, tag=2),
-               # receives in the peer's send order (its to_left arrives "from right"): NCCL matches by order, not tag
-               dist.P2POp(dist.irecv, n_in[1:2], right, self.group, tag=1), dist.P2POp(dist.irecv, n_in[0:1], left, self.group, tag=2)]
-        for r in dist.batch_isend_irecv(ops):
-            r.wait()
-        n_l, n_r = int(n_in[0]), int(n_in[1])
-        recv = [torch.empty((n_l, c), dtype=torch.float64, device=cdev), torch.empty((n_r, c), dtype=torch.float64, device=cdev)]
-        ops = []
-        if send[0].shape[0]:
-            ops.append(dist.P2POp(dist.isend, send[0], left, self.group, tag=3))
-        if send[1].shape[0]:
-            ops.append(dist.P2POp(dist.isend, send[1], right, self.group, tag=4))
-        if n_r:
-            ops.append(dist.P2POp(dist.irecv, recv[1], right, self.group, tag=3))
-        if n_l:
-            ops.append(dist.P2POp(dist.irecv, recv[0], left, self.group, tag=4))
-        if ops:
-            for r in dist.batch_isend_irecv(ops):
-                r.wait()
-        self.bytes_sent += 8 * c * (send[0].shape[0] + send[1].shape[0])
-        return recv[0].to(dev), recv[1].to(dev)
-
-    def _halo(self, with_dynamics: bool):
-        """Ghost copies (global coordinates) of the neighbours' atoms within g of my slab."""
-        dev = self.engine.device
-        n = self.pos.shape[0]
-        if self.world == 1:
-            z = torch.zeros((0, 3), dtype=torch.float64, device=dev)
-            return z, z, z, torch.zeros(0, dtype=torch.int32, device=dev)
-        x = self.pos[:, self.axis] - self.lo
-        cols = [self.pos, self.types.to(torch.float64).reshape(n, 1)]
-        if with_dynamics:
-            cols += [self.vel, self.frc]
-        payload = torch.cat(cols, dim=1)
-        got_l, got_r = self._exchange(payload[x < self.g], payload[x >= self.w - self.g])
-        got = torch.cat([got_l, got_r], dim=0)
-        gpos, gtyp = got[:, 0:3], got[:, 3].to(torch.int32)
-        if with_dynamics:
-            return gpos, got[:, 4:7], got[:, 7:10], gtyp
-        z = torch.zeros_like(gpos)
-        return gpos, z, z, gtyp
-
-    def _migrate(self):
-        """Hand owned atoms that left the slab to the neighbour that now owns them."""
-        if self.world == 1:
-            return
-        n = self.pos.shape[0]
-        owner = self.owner_of(self.pos[:, self.axis])
-        left, right = (self.rank - 1) % self.world, (self.rank + 1) % self.world
-        stay = owner == self.rank
-        go_l = (owner == left) & ~stay
-        go_r = (owner == right) & ~stay & ~go_l
-        if bool((~(stay | go_l | go_r)).any()):
-            raise RuntimeError("an atom moved further than one slab in one step")
-        payload = torch.cat([self.pos, self.vel, self.frc, self.types.to(torch.float64).reshape(n, 1),
-                             self.gid.to(torch.float64).reshape(n, 1), self.E.reshape(n, 1),
-                             (self.V if self.V is not None else torch.zeros_like(self.E)).reshape(n, 1)], dim=1)
-        got_l, got_r = self._exchange(payload[go_l], payload[go_r])
-        allp = torch.cat([payload[stay], got_l, got_r], dim=0)
-        self.pos, self.vel, self.frc = allp[:, 0:3].contiguous(), allp[:, 3:6].contiguous(), allp[:, 6:9].contiguous()
-        self.types, self.gid = allp[:, 9].to(torch.int32), allp[:, 10].to(torch.int64)
-        self.E = allp[:, 11].contiguous()
-        self.V = allp[:, 12].contiguous() if self.V is not None else None
-
-    # ------------------------------------------------------------------ the two entry points
-    def compute(self, variances: bool = False):
-        """One distributed force-field evaluation: E, F, V of the owned atoms (also kept as the MD forces)."""
-        gpos, _, _, gtyp = self._halo(False)
-        n = self.pos.shape[0]
-        lpos = self._to_local(torch.cat([self.pos, gpos], dim=0))
-        ltyp = torch.cat([self.types, gtyp], dim=0)
-        e, f, v = self.engine.evaluate(lpos, ltyp, self.local_box, self.local_pbc, variances)
-        self.E, self.frc = e[:n].clone(), f[:n].clone()
-        self.V = v[:n].clone() if v is not None else None
-        return self.E, self.frc, self.V
-
-    def step(self, dt: float, n_steps: int = 1, variances: bool = False):
-        """n_steps of velocity Verlet on the decomposed system."""
-        if self.frc is None:
-            self.compute(variances)
-        for _ in range(n_steps):
-            gpos, gvel, gfrc, gtyp = self._halo(True)
-            n = self.pos.shape[0]
-            lpos = self._to_local(torch.cat([self.pos, gpos], dim=0))
-            lvel = torch.cat([self.vel, gvel], dim=0)
-            lfrc = torch.cat([self.frc, gfrc], dim=0)
-            ltyp = torch.cat([self.types, gtyp], dim=0)
-            p, v, e, f, var = self.engine.md_step(lpos, lvel, lfrc, ltyp, self.local_box, self.local_pbc, dt, variances)
-            self.pos = self._to_global(p[:n]) if self.world > 1 else p[:n].clone()
-            self.vel, self.frc, self.E = v[:n].clone(), f[:n].clone(), e[:n].clone()
-            self.V = var[:n].clone() if var is not None else None
-            self._migrate()
-        return self
-
-    # ------------------------------------------------------------------ collect (tests, output)
-    def gather(self):
-        """Rank 0 gets dict(pos, vel, F, E, V, types) of the whole system in the original atom order; others None."""
-        n = self.pos.shape[0]
-        V = self.V if self.V is not None else torch.zeros(n, dtype=torch.float64, device=self.pos.device)
-        E = self.E if self.E is not None else torch.zeros(n, dtype=torch.float64, device=self.pos.device)
-        F = self.frc if self.frc is not None else torch.zeros_like(self.pos)
-        mine = torch.cat([self.gid.to(torch.float64).reshape(n, 1), self.pos, self.vel, F, E.reshape(n, 1), V.reshape(n, 1),
-                          self.types.to(torch.float64).reshape(n, 1)], dim=1).cpu()
+    def gather(self, variances: bool = True):
+        """Rank 0 gets dict(pos, vel, F, E, V, types-free) of the whole system in the original atom order; others None."""
+        o = self.engine.owned(variances)
+        pos = o["pos"] + self.lo[None, :]
+        for ph in self.phases:
+            a, Lx = ph["axis"], self.L[ph["axis"]]
+            pos[:, a] -= Lx * np.floor(pos[:, a] / Lx)
+        mine = dict(tags=o["tags"], pos=pos, vel=o["vel"], E=o["E"], F=o["F"],
+                    V=o["V"] if o["V"] is not None else np.zeros(len(pos)))
         if self.world == 1:
             parts = [mine]
         else:
             parts = [None] * self.world
-            dist.all_gather_object(parts, mine.numpy(), group=self.group)
-            parts = [torch.as_tensor(p) for p in parts]
+            dist.all_gather_object(parts, mine, group=self.group)
         if self.rank != 0:
             return None
-        allp = torch.cat(parts, dim=0).numpy()
-        order = np.argsort(allp[:, 0].astype(np.int64), kind="stable")
-        a = allp[order]
-        assert np.array_equal(a[:, 0].astype(np.int64), np.arange(a.shape[0])), "atoms lost or duplicated"
-        return dict(pos=a[:, 1:4], vel=a[:, 4:7], F=a[:, 7:10], E=a[:, 10], V=a[:, 11], types=a[:, 12].astype(np.int32))
+        tags = np.concatenate([p["tags"] for p in parts])
+        order = np.argsort(tags, kind="stable")
+        assert np.array_equal(tags[order], np.arange(len(tags))), "atoms lost or duplicated"
+        return {k: np.concatenate([p[k] for p in parts])[order] for k in ("pos", "vel", "E", "F", "V")}
+
+    # ------------------------------------------------------------------ messages
+    def _new_msg(self, rows, width):
+        return torch.zeros(MSG_HEADER + rows * width, dtype=torch.float64, device=self.engine.device)
+
+    def _exchange(self, ph, out_lo, out_hi, in_lo, in_hi):
+        """Send out_lo to the lo neighbour and out_hi to the hi neighbour; receive in_lo from lo, in_hi from hi.
+        Sizes are known on both sides.  gloo (CPU tests) stages through host memory."""
+        lo, hi = ph["lo_rank"], ph["hi_rank"]
+        if ph["p"] == 1:  # self-exchange: what I send towards hi arrives from my lo side
+            in_lo.copy_(out_hi)
+            in_hi.copy_(out_lo)
+            return
+        host = dist.get_backend(self.group) == "gloo" and self.engine.device.type != "cpu"
+        so, si = ([t.cpu() for t in (out_lo, out_hi)], [torch.empty_like(t, device="cpu") for t in (in_lo, in_hi)]) if host \
+            else ([out_lo, out_hi], [in_lo, in_hi])
+        # receives in the peer's send order (with two ranks along the axis both messages come from the same peer, its
+        # to-lo first: that one arrives "from hi"): NCCL matches by order, not by tag
+        ops = [dist.P2POp(dist.isend, so[0], lo, self.group, tag=1), dist.P2POp(dist.isend, so[1], hi, self.group, tag=2),
+               dist.P2POp(dist.irecv, si[1], hi, self.group, tag=1), dist.P2POp(dist.irecv, si[0], lo, self.group, tag=2)]
+        for r in dist.batch_isend_irecv(ops):
+            r.wait()
+        if host:
+            in_lo.copy_(si[0])
+            in_hi.copy_(si[1])
+        self.bytes_sent += 8 * (out_lo.numel() + out_hi.numel())
+
+    # ------------------------------------------------------------------ rebuild
+    def rebuild(self):
+        """Migration, new send lists, new ghost shell; one synchronisation at the end (the new local atom count)."""
+        e = self.engine
+        mcap, bcap = self.migrate_capacity, self.border_capacity
+        for ph in self.phases:
+            out_lo, out_hi = self._new_msg(mcap, MSG_FULL_ROW), self._new_msg(mcap, MSG_FULL_ROW)
+            in_lo, in_hi = self._new_msg(mcap, MSG_FULL_ROW), self._new_msg(mcap, MSG_FULL_ROW)
+            e.migrate_pack(ph["axis"], self.h, self.h + ph["w"], ph["w"], -ph["w"], out_lo, out_hi, mcap)
+            self._exchange(ph, out_lo, out_hi, in_lo, in_hi)
+            e.migrate_unpack(in_lo, in_hi, mcap)
+        inf = float("inf")
+        for k, ph in enumerate(self.phases):
+            out_lo, out_hi = self._new_msg(bcap, MSG_FULL_ROW), self._new_msg(bcap, MSG_FULL_ROW)
+            in_lo, in_hi = self._new_msg(bcap, MSG_FULL_ROW), self._new_msg(bcap, MSG_FULL_ROW)
+            e.border_pack(k, ph["axis"], -inf, 2.0 * self.h, ph["w"], inf, ph["w"], -ph["w"], out_lo, out_hi, bcap)
+            self._exchange(ph, out_lo, out_hi, in_lo, in_hi)
+            e.border_unpack(k, in_lo, in_hi, bcap)
+        self.counts = e.commit()
+        c = self.counts
+        self._fwd = [dict(out_lo=self._new_msg(c["send"][2 * k], MSG_FWD_ROW), out_hi=self._new_msg(c["send"][2 * k + 1], MSG_FWD_ROW),
+                          in_lo=self._new_msg(c["recv"][2 * k], MSG_FWD_ROW), in_hi=self._new_msg(c["recv"][2 * k + 1], MSG_FWD_ROW))
+                     for k in range(len(self.phases))]
+        self.built = True
+        self.rebuilds += 1
+        self._flags.clear()  # signals raised before this rebuild are stale
+
+    def _forward(self):
+        for k, ph in enumerate(self.phases):
+            m = self._fwd[k]
+            self.engine.forward_pack(k, m["out_lo"], m["out_hi"])
+            self._exchange(ph, m["out_lo"], m["out_hi"], m["in_lo"], m["in_hi"])
+            self.engine.forward_unpack(k, m["in_lo"], m["in_hi"])
+
+    # ------------------------------------------------------------------ rebuild signal (asynchronous, lagged)
+    def _post_signal(self):
+        dev = self.engine.device
+        flag = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.engine.signal(flag)
+        if self.world > 1:
+            if dist.get_backend(self.group) == "gloo" and dev.type != "cpu":
+                f = flag.cpu()
+                dist.all_reduce(f, op=dist.ReduceOp.MAX, group=self.group)
+                flag = f
+            else:
+                dist.all_reduce(flag, op=dist.ReduceOp.MAX, group=self.group)
+        if flag.is_cuda:
+            host = torch.empty(1, dtype=torch.int32, pin_memory=True)
+            host.copy_(flag, non_blocking=True)
+            ev = torch.cuda.Event()
+            ev.record()
+            self._flags.append((host, ev))
+        else:
+            self._flags.append((flag, None))
+
+    def _signal_due(self) -> bool:
+        """The flag posted `lag` steps ago (identical on all ranks); waiting on it does not stall the GPU."""
+        if len(self._flags) < self.lag:
+            return False
+        host, ev = self._flags.popleft()
+        if ev is not None:
+            ev.synchronize()
+        return bool(int(host[0]) != 0)
+
+    # ------------------------------------------------------------------ the two entry points
+    def compute(self, variances: bool = False):
+        """Forces, energies (and variances) of the current positions on every rank's owned atoms."""
+        if not self.built:
+            self.rebuild()
+        self._forward()
+        self.engine.step(0.0, 0, variances)
+        return self
+
+    def step(self, dt: float, n_steps: int = 1, variances: bool = False):
+        """n_steps of velocity Verlet on the decomposed system."""
+        if not self.built:
+            self.compute(variances)
+        for _ in range(n_steps):
+            if self.phases and self._signal_due():
+                self.rebuild()
+            self._forward()
+            self.engine.step(dt, 1, variances)
+            if self.phases:
+                self._post_signal()
+        return self
