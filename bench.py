@@ -15,9 +15,10 @@ the line reports the MEDIAN repeat and lists all of them.  At N
 `roofline` (the dominant kernel), `roofline_kernels` (every phase against its own bound), `sweep` (configs 1, 2, 4 and
 the six runs of config 5, short step counts) and `cpu_baseline` (the oracle on the host cores, all cores and 1 thread).
 
-For N > 1 (launched by torch.distributed.run) the ranks share ONE system N times as long as the workload, cut into
-N domains with a halo exchange per step (paper_2204_12573_b200/halo.py; `--replicas` runs N independent copies
-instead); value = all ranks' atom-steps / max-over-ranks device time.  Prints ONE JSON line on rank 0.
+For N > 1 (launched by torch.distributed.run) the ranks share ONE slab px x py times the C3 cell, one C3-sized domain
+per GPU on a 2-D process grid with a halo exchange per step (paper_2204_12573_b200/halo.py + the device data plane
+flare_domain_*; `--replicas` runs N independent copies instead); value = all ranks' atom-steps / max-over-ranks device
+time.  `--decomposed` at N = 1 runs the same path with the rank as its own neighbour.  Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
 
@@ -312,14 +313,24 @@ def kernel_rooflines(ctx, s, res, want_var, peaks, steps):
 # ----------------------------------------------------------------------------- GPU arm, decomposed (N > 1)
 
 
+def process_grid(world: int):
+    """Near-square px x py factorisation, px >= py (the slab is near-two-dimensional)."""
+    py = int(np.floor(np.sqrt(world)))
+    while world % py:
+        py -= 1
+    return world // py, py
+
+
 def run_decomposed(args):
-    """Weak scaling of the real multi-GPU path: one H2/Pt(111) slab `world` times as long as C3 along x, cut into
-    `world` domains, halo exchange every step (NCCL point-to-point).  Same JSON line; roofline / cpu_baseline omitted."""
+    """Weak scaling of the real multi-GPU path: one H2/Pt(111) slab px x py times the C3 cell, one C3-sized domain
+    per GPU on a 2-D process grid, device data plane (flare_domain_*), one halo exchange per step over
+    torch.distributed point-to-point (NCCL).  At N = 1 the rank is its own neighbour on all four sides (self-halo), so
+    the same kernels and messages run.  Same JSON line; roofline / cpu_baseline belong to the N = 1 plain run."""
     import torch
     import torch.distributed as dist
 
     from paper_2204_12573_b200 import flare
-    from paper_2204_12573_b200.halo import CudaEngine, SlabDecomposition
+    from paper_2204_12573_b200.halo import CudaEngine, DomainDecomposition
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -328,10 +339,18 @@ def run_decomposed(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     want_var = not args.no_variance
-    s = workloads.h2_pt111_config(3, 408 * world, 204, 41616 * world, name=f"C3x{world}")
-    ctx = flare.from_system(s, device=local, variance=want_var)
-    eng = CudaEngine(ctx, capacity=int(1.2 * s.n_atoms / world) + 4096)
-    dd = SlabDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), axis=0).scatter(s.pos, s.vel, s.types)
+    px, py = process_grid(world)
+    nx, ny, nh2 = (408, 204, 41616) if args.workload != "tile" else (48, 24, 576)
+    s = workloads.h2_pt111_config(3, nx * px, ny * py, nh2 * world, name=f"C3x{px}x{py}")
+    ctx = flare.from_system(s, device=local, variance=want_var, timing=True)
+    rc_max = float(np.max(s.r_cut))
+    halo_skin = 6.0  # domains are ~1000 A wide: a thick ghost shell is cheap (0.4 % more atoms per A) and spaces the rebuilds
+    Lx, Ly = float(s.box[0]), float(s.box[4])
+    h = 2.0 * rc_max + halo_skin
+    shell = (1.0 + 2.0 * h / (Lx / px)) * (1.0 + 2.0 * h / (Ly / py))
+    eng = CudaEngine(ctx, capacity=int(1.1 * shell * s.n_atoms / world) + 65536)
+    dd = DomainDecomposition(eng, s.box, s.pbc, rc_max, grid=(px, py), halo_skin=halo_skin, self_halo=(world == 1))
+    dd.scatter(s.pos, s.vel, s.types)
     dt_fs = float(s.meta.get("dt_fs", 0.5))
     dd.compute(want_var)
 
@@ -341,34 +360,47 @@ def run_decomposed(args):
         torch.cuda.synchronize()
 
     dd.step(dt_fs, args.warmup, want_var)
-    launches0 = ctx.kernel_launches()
-    sent0 = dd.bytes_sent
+    reps = []
     sampler = ClockSampler(local)
-    barrier()
-    if rank == 0:
-        sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    dd.step(dt_fs, args.steps, want_var)
-    ev1.record()
-    barrier()
+    for rep in range(args.repeats):
+        launches0, sent0, rebuilds0 = ctx.kernel_launches(), dd.bytes_sent, dd.rebuilds
+        ctx.timings()
+        barrier()
+        if rank == 0 and rep == 0:
+            sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        dd.step(dt_fs, args.steps, want_var)
+        ev1.record()
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=torch.device("cuda", local))
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        reps.append({"ms_total": ms, "launches": ctx.kernel_launches() - launches0, "bytes": dd.bytes_sent - sent0,
+                     "rebuilds": dd.rebuilds - rebuilds0, "phases": ctx.timings()})
     clocks = sampler.stop() if rank == 0 else {}
-    ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=torch.device("cuda", local))
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ctx.check()
+    order = sorted(range(len(reps)), key=lambda r: reps[r]["ms_total"])
+    med = reps[order[len(reps) // 2]]
     if rank == 0:
         line = {
-            "metric": METRIC, "value": s.n_atoms * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "metric": METRIC, "value": s.n_atoms * args.steps / (med["ms_total"] * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": med["ms_total"] / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"C3 construction {world}x as long along x: {s.n_atoms} atoms on {world} slab(s), "
-                                   "halo 2 r_cut, one exchange + one migration per step", "atoms": s.n_atoms, "P": s.P,
-                       "variance": want_var, "dt_fs": dt_fs, "parallelism": f"slab decomposition x{world}",
-                       "halo_bytes_per_rank_per_step": (dd.bytes_sent - sent0) / max(1, args.steps),
+            "repeats": len(reps), "repeats_ms_per_step": [r["ms_total"] / args.steps for r in reps],
+            "config": {"workload": f"C3 construction tiled {px} x {py}: {s.n_atoms} atoms, one C3-sized domain per GPU on a "
+                                   f"{px} x {py} process grid, halo 2 r_cut + {halo_skin} A, device data plane, one exchange per step"
+                                   + (" (N = 1: self-halo, the rank is its own neighbour)" if world == 1 else ""),
+                       "atoms": s.n_atoms, "P": s.P, "variance": want_var, "dt_fs": dt_fs,
+                       "parallelism": f"domain decomposition {px}x{py}",
+                       "owned_atoms_rank0": dd.counts["n_owned"], "local_atoms_rank0": dd.counts["n_local"],
+                       "halo_bytes_per_rank_per_step": med["bytes"] / max(1, args.steps),
+                       "rebuilds_in_window": med["rebuilds"], "candidate_list_rebuilds_total_rank0": ctx.get_option(6),
                        "l2": "working set far larger than L2; no flush needed"},
-            "clocks": clocks, "gpu_launches": ctx.kernel_launches() - launches0,
+            "phases_ms_per_step_rank0": {k: v[0] / args.steps for k, v in med["phases"].items()},
+            "clocks": clocks, "gpu_launches": med["launches"],
         }
         print(json.dumps(line))
     if world > 1:
@@ -636,14 +668,15 @@ def main():
                     help="also run flare_analyze (maximum uncertainty + H-H coordination within 1 A) after every step "
                          "inside the timed region, like the paper's production run (P:L247-249)")
     ap.add_argument("--decomposed", action="store_true",
-                    help="N ranks share ONE system N times as long as C3 (slab decomposition + halo exchange, "
-                         "paper_2204_12573_b200/halo.py) instead of running N replicas")
+                    help="run the multi-GPU path (2-D domain decomposition + halo exchange through the device data plane, "
+                         "paper_2204_12573_b200/halo.py): the default for N > 1; at N = 1 the rank is its own neighbour")
+    ap.add_argument("--replicas", action="store_true", help="N > 1: N independent replicas of the workload instead")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     args.repeats = max(1, args.repeats)
     if args.impl == "reference":
         run_reference(args)
-    elif args.decomposed:
+    elif args.decomposed or (int(os.environ.get("WORLD_SIZE", "1")) > 1 and not args.replicas):
         run_decomposed(args)
     else:
         run_ours(args)

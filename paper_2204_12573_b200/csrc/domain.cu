@@ -82,10 +82,10 @@ __global__ void __launch_bounds__(1024) k_dom_scan(int nb, int* __restrict__ blk
     }
 }
 
-// ordered write of the three index lists (any may be null); entries beyond `cap` are dropped and flagged
+// ordered write of the three index lists (any may be null); entries beyond `cap` (`cap_stay`) are dropped and flagged
 __global__ void __launch_bounds__(kDomBlock)
 k_dom_write(DomSel s, const int* __restrict__ dom, const double* __restrict__ x, const int* __restrict__ blk,
-            int* __restrict__ list_lo, int* __restrict__ list_hi, int* __restrict__ list_stay, int cap,
+            int* __restrict__ list_lo, int* __restrict__ list_hi, int* __restrict__ list_stay, int cap, int cap_stay,
             int* __restrict__ flags) {
     __shared__ int wcnt[3][32];
     const int n = dom[s.n_from];
@@ -117,7 +117,7 @@ k_dom_write(DomSel s, const int* __restrict__ dom, const double* __restrict__ x,
     for (int r = 0; r < 3; r++) {
         if (in[r] && lists[r]) {
             const int pos = blk[r * nb + blockIdx.x] + wcnt[r][warp] + __popc(bal[r] & ((1u << lane) - 1u));
-            if (pos < cap) lists[r][pos] = i;
+            if (pos < (r == 2 ? cap_stay : cap)) lists[r][pos] = i;
             else atomicOr(flags, kFlagDomainOverflow);
         }
     }
@@ -189,6 +189,7 @@ __global__ void k_dom_gather_stay(const int* __restrict__ list, const int* __res
                                   const double* __restrict__ v, const double* __restrict__ f,
                                   const int* __restrict__ types, const long long* __restrict__ tag,
                                   double* __restrict__ tmp /*[n][11]*/) {
+    if (dom[kDomTot] + dom[kDomTot + 1] == 0) return;  // nobody leaves: the atoms that stay are already in place
     const int cnt = dom[kDomTot + 2];
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < cnt; r += gridDim.x * blockDim.x) {
         const size_t i = (size_t)list[r];
@@ -202,6 +203,7 @@ __global__ void k_dom_gather_stay(const int* __restrict__ list, const int* __res
 __global__ void k_dom_scatter_stay(const int* __restrict__ dom, const double* __restrict__ tmp, double* __restrict__ x,
                                    double* __restrict__ v, double* __restrict__ f, int* __restrict__ types,
                                    long long* __restrict__ tag) {
+    if (dom[kDomTot] + dom[kDomTot + 1] == 0) return;
     const int cnt = dom[kDomTot + 2];
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < cnt; r += gridDim.x * blockDim.x) {
         const double* row = tmp + (size_t)r * kDomFullRow;
@@ -247,13 +249,13 @@ __global__ void k_dom_unpack_fwd(const double* __restrict__ msg, int off, int cn
 static int dom_grid(int n) { return std::max(1, std::min((n + 255) / 256, 148 * 8)); }
 
 void dom_select(Launcher& L, const Workspace& ws, const DomSel& s, int n_bound, int* list_lo, int* list_hi,
-                int* list_stay, int cap) {
+                int* list_stay, int cap) {  // the stay list (if any) holds up to n_bound entries
     const int nb = std::max(1, (n_bound + kDomBlock - 1) / kDomBlock);
     int* blk = ws.cell_cnt;  // scratch (free between evaluations): 3 nb ints
     L.launch(k_dom_count, dim3(nb), dim3(kDomBlock), 0, s, (const int*)ws.dom, (const double*)ws.x, blk);
     L.launch(k_dom_scan, dim3(1), dim3(1024), 0, nb, blk, ws.dom);
     L.launch(k_dom_write, dim3(nb), dim3(kDomBlock), 0, s, (const int*)ws.dom, (const double*)ws.x, (const int*)blk,
-             list_lo, list_hi, list_stay, cap, ws.flags);
+             list_lo, list_hi, list_stay, cap, n_bound, ws.flags);
 }
 
 void dom_commit_lists(Launcher& L, const Workspace& ws, int slot_lo, int slot_hi, int cap) {

@@ -352,6 +352,7 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.tag = cv.take<long long>(N);
     w.dom = cv.take<int>(kDomInts);
     w.send_idx = cv.take<int>(4 * (N / 2 + 1024));
+    w.dom_ref = cv.take<double>(3 * N);
     if (ws) *ws = w;
     if (chunk_out) *chunk_out = chunk;
     if (cells_out) *cells_out = (int)std::min<size_t>(cells, 0x7fffffff);
@@ -1009,6 +1010,8 @@ int flare_domain_commit(flare_ctx* c, int64_t counts[14]) {
         c->dom_recv_off[q] = h[kDomRecvOff + q];
     }
     FLARE_CUDA(c, cudaMemsetAsync(c->ws.dom + kDomNeed, 0, sizeof(int), c->stream));
+    if (c->n > 0)  // displacements are measured from here on
+        FLARE_CUDA(c, cudaMemcpyAsync(c->ws.dom_ref, c->ws.x, sizeof(double) * 3 * (size_t)c->n, cudaMemcpyDeviceToDevice, c->stream));
     c->list_valid = false;  // membership changed: the candidate list is rebuilt by the next evaluation
     c->pairf_valid = false;
     drop_step_graph(c);

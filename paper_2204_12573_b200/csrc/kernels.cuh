@@ -201,6 +201,7 @@ struct Workspace {
     long long* tag = nullptr;  // [N] global atom id (travels with the atom)
     int* dom = nullptr;        // [kDomInts] counters, see kDom*
     int* send_idx = nullptr;   // [4][N/2 + 1024] send lists of the two exchange phases
+    double* dom_ref = nullptr; // [N][3] positions at the last domain rebuild (caller order)
 };
 constexpr int kRedBlocksMax = 1184;
 

@@ -402,7 +402,8 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
 // build (as the bits of a float rounded up: non-negative floats order like their bit patterns) -> dmax[S]
 __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, const int* __restrict__ types,
                           const int* __restrict__ order, const AtomS* __restrict__ ref, AtomS* __restrict__ atoms,
-                          int* __restrict__ gate, int* __restrict__ dmax, int* __restrict__ flags) {
+                          int* __restrict__ gate, int* __restrict__ dmax, int* __restrict__ flags,
+                          const double* __restrict__ dom_ref, double dom_trigger2, int* __restrict__ dom_need) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     int my_type = -1;
     int bits = 0;
@@ -414,6 +415,19 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
         for (int d = 0; d < 3; d++) {
             if (!isfinite(p[d])) { bad = true; p[d] = 0.0; }
             if (g.pbc[d]) p[d] = wrap_coord(p[d], g.L[d]);
+        }
+        if (dom_ref) {
+            // domain decomposition (domain.cu): the ghost shell was chosen for the positions of the last domain rebuild
+            // and tolerates a displacement of dom_trigger per atom, whatever the candidate list did in between
+            double d2 = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                double r = dom_ref[3 * (size_t)i + d];
+                if (g.pbc[d]) r = wrap_coord(r, g.L[d]);
+                const double dd = min_image(p[d] - r, g.L[d], g.half[d], g.pbc[d]);
+                d2 += dd * dd;
+            }
+            if (!(d2 < dom_trigger2)) *dom_need = 1;  // benign race: every writer stores 1
         }
         AtomS a;
         a.x = p[0]; a.y = p[1]; a.z = p[2];
@@ -446,14 +460,9 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
 // rebuilds.  The threshold is taken a hair low so that the triangle inequality holds with rounding to spare.
 // In a captured step (CUDA graph, small systems) the decision also drives the IF node that holds the rebuild chain.
 __global__ void k_gate_decide(Basis bs, double reach, const int* __restrict__ dmax, int* __restrict__ gate,
-                              cudaGraphConditionalHandle cond, int use_cond, float dom_trigger, int* __restrict__ dom_need) {
+                              cudaGraphConditionalHandle cond, int use_cond) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     int need = *gate;  // k_refresh raises it for a non-finite position or a changed species
-    if (dom_need) {  // domain decomposition: the ghost shell has dom_trigger of slack per atom (domain.cu)
-        float m = 0.f;
-        for (int a = 0; a < bs.S; a++) m = fmaxf(m, __int_as_float(dmax[a]));
-        if (m >= dom_trigger || need) *dom_need = 1;
-    }
     for (int a = 0; a < bs.S; a++)
         for (int b = a; b < bs.S; b++) {
             const double da = __int_as_float(dmax[a]), db = __int_as_float(dmax[b]);
@@ -676,13 +685,15 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
         if (list_valid) {
             L.memset(ws.skin_gate + 4, 0, sizeof(int) * kMaxSpecies);  // per-species maximum displacement
             L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, bs.S, n, pos, types, (const int*)ws.order,
-                     (const AtomS*)ws.ref, ws.atoms, ws.skin_gate, ws.skin_gate + 4, ws.flags);
+                     (const AtomS*)ws.ref, ws.atoms, ws.skin_gate, ws.skin_gate + 4, ws.flags,
+                     dom_trigger > 0.0 ? (const double*)ws.dom_ref : (const double*)nullptr, dom_trigger * dom_trigger,
+                     ws.dom + kDomNeed);
             // captured step: the rebuild chain below becomes the body of an IF node that k_gate_decide switches on,
             // so a step that keeps its list pays for none of the chain's (otherwise empty) launches
             const bool as_if = L.capturing;
             const cudaGraphConditionalHandle h = as_if ? L.cond_handle() : 0;
             L.launch(k_gate_decide, dim3(1), dim3(32), 0, bs, reach, (const int*)(ws.skin_gate + 4), ws.skin_gate, h,
-                     as_if ? 1 : 0, (float)dom_trigger, dom_trigger > 0.0 ? ws.dom + kDomNeed : (int*)nullptr);
+                     as_if ? 1 : 0);
             if (as_if) { L.begin_if(h); gate = nullptr; }
         }
     }

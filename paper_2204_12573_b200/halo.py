@@ -24,7 +24,7 @@ STEP (between rebuilds; nothing blocks the host): forward rows (x, v, F) of the 
 `flare_step(dt, 1)` on owned + ghosts (ghosts carry their owner's velocity and force, so the integrator moves them as
 their owner does), rebuild signal.  Membership, order and counts are stable between rebuilds, so the context's
 candidate neighbour list survives.  The signal -- "some atom has moved `trigger` since the rebuild", raised on the
-device by the same kernel that gates the candidate list -- is all-reduced (MAX) asynchronously and read `lag` steps
+device by the kernel that refreshes the candidate list -- is all-reduced (MAX) asynchronously and read `lag` steps
 later, so every rank takes the same decision without a per-step host synchronisation; the halo skin covers
 2 x trigger plus the motion of those `lag` steps (trigger = 0.35 halo_skin).
 """
@@ -65,7 +65,6 @@ class CudaEngine(Engine):
         self.device = flare_ctx.device
         self.capacity = int(capacity)
         self.ctx.bind(self.capacity)
-        self.skin = 1e-3 * self.ctx.get_option(5)  # FLARE_OPT_SKIN_MILLI_ANGSTROM
         self.n_owned = 0
 
     def begin(self, pos, vel, types, tags, box, pbc, trigger):
@@ -124,10 +123,6 @@ class DomainDecomposition:
         self.pbc = np.asarray(pbc, dtype=np.int32).reshape(3).copy()
         self.h = 2.0 * float(r_cut_max) + float(halo_skin)
         self.trigger = 0.35 * float(halo_skin)
-        # the engine's own candidate list may restart the displacement tracking when ITS skin is used up (that raises the
-        # signal too); until the rebuild `lag` steps later an atom may have moved that skin: it must fit into half the halo skin
-        if getattr(engine, "skin", 0.0) > 0.4 * float(halo_skin):
-            raise ValueError(f"halo_skin {halo_skin} must be at least 2.5 x the engine's list skin {engine.skin}")
         self.lag = max(1, int(lag))
         coords = (self.rank // grid[1], self.rank % grid[1])
         # decomposed axes = exchange phases, in order
@@ -162,6 +157,7 @@ class DomainDecomposition:
         self.bytes_sent = 0
         self._flags = collections.deque()
         self._fwd = None
+        self._rb = None
 
     # ------------------------------------------------------------------ initial distribution and collection (I/O)
     def scatter(self, pos, vel, types):
@@ -221,6 +217,7 @@ class DomainDecomposition:
         if ph["p"] == 1:  # self-exchange: what I send towards hi arrives from my lo side
             in_lo.copy_(out_hi)
             in_hi.copy_(out_lo)
+            self.bytes_sent += 8 * (out_lo.numel() + out_hi.numel())
             return
         host = dist.get_backend(self.group) == "gloo" and self.engine.device.type != "cpu"
         so, si = ([t.cpu() for t in (out_lo, out_hi)], [torch.empty_like(t, device="cpu") for t in (in_lo, in_hi)]) if host \
@@ -241,16 +238,16 @@ class DomainDecomposition:
         """Migration, new send lists, new ghost shell; one synchronisation at the end (the new local atom count)."""
         e = self.engine
         mcap, bcap = self.migrate_capacity, self.border_capacity
+        if self._rb is None and self.phases:  # the fixed-capacity rebuild messages are allocated once
+            self._rb = {k: [self._new_msg(cap, MSG_FULL_ROW) for _ in range(4)] for k, cap in (("m", mcap), ("b", bcap))}
         for ph in self.phases:
-            out_lo, out_hi = self._new_msg(mcap, MSG_FULL_ROW), self._new_msg(mcap, MSG_FULL_ROW)
-            in_lo, in_hi = self._new_msg(mcap, MSG_FULL_ROW), self._new_msg(mcap, MSG_FULL_ROW)
+            out_lo, out_hi, in_lo, in_hi = self._rb["m"]
             e.migrate_pack(ph["axis"], self.h, self.h + ph["w"], ph["w"], -ph["w"], out_lo, out_hi, mcap)
             self._exchange(ph, out_lo, out_hi, in_lo, in_hi)
             e.migrate_unpack(in_lo, in_hi, mcap)
         inf = float("inf")
         for k, ph in enumerate(self.phases):
-            out_lo, out_hi = self._new_msg(bcap, MSG_FULL_ROW), self._new_msg(bcap, MSG_FULL_ROW)
-            in_lo, in_hi = self._new_msg(bcap, MSG_FULL_ROW), self._new_msg(bcap, MSG_FULL_ROW)
+            out_lo, out_hi, in_lo, in_hi = self._rb["b"]
             e.border_pack(k, ph["axis"], -inf, 2.0 * self.h, ph["w"], inf, ph["w"], -ph["w"], out_lo, out_hi, bcap)
             self._exchange(ph, out_lo, out_hi, in_lo, in_hi)
             e.border_unpack(k, in_lo, in_hi, bcap)
