@@ -348,7 +348,7 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.red = cv.take<double>((size_t)kRedBlocksMax * 9);
     w.scal = cv.take<double>(16);
     w.ascal = cv.take<unsigned long long>(18);
-    w.qf_counter = cv.take<int>(kMaxGroups);
+    w.qf_counter = cv.take<int>(3 * kMaxGroups);
     w.tag = cv.take<long long>(N);
     w.dom = cv.take<int>(kDomInts);
     w.send_idx = cv.take<int>(4 * (N / 2 + 1024));

@@ -196,7 +196,7 @@ struct Workspace {
     double* red = nullptr;                 // [kRedBlocksMax][9] per-block partial sums
     double* scal = nullptr;                // [16]: [0..8] virial, [12..15] thermostat xi, eta, scale, K2
     unsigned long long* ascal = nullptr;   // [18] analysis outputs (max bits, count, coordination histogram)
-    int* qf_counter = nullptr;             // [kMaxGroups] tile queues of the quadratic-form launches
+    int* qf_counter = nullptr;             // [3 kMaxGroups] tile / block queues of the quadratic-form launches
     // ---- domain decomposition
     long long* tag = nullptr;  // [N] global atom id (travels with the atom)
     int* dom = nullptr;        // [kDomInts] counters, see kDom*

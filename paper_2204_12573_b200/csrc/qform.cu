@@ -15,6 +15,8 @@
 // sum_n W[r][n] B[r][n]; variance tiles store only the partial row-dot.  Partials of the ntn tiles
 // of a row are summed in fixed order by the back-propagation kernel (deterministic, atomics-free).
 // The rows hold the UNNORMALISED B; the 1/||B||^2 factor is applied by the back-propagation kernel.
+#include <algorithm>
+
 #include "kernels.cuh"
 
 namespace flare {
@@ -283,12 +285,230 @@ static void launch_qform(Launcher& L, const QfArgs& a, int sm_count, long long m
     L.launch(k_qform<NB, WARPS>, dim3(grid), dim3(C::THREADS), smem, a);
 }
 
+// ------------------------------------------------------------------ K <= 144: matrix resident in shared memory
+// For the small matrices (P = 144 after the species-sparse compaction: 98 % of the rows of the H2/Pt(111)
+// workloads) the whole symmetric matrix fits in one SM's shared memory (144 x 148 doubles = 170 KB).  One persistent
+// CTA per SM keeps ONE matrix (beta or Sigma) resident -- fetched once by per-row bulk copies (TMA, completion on an
+// mbarrier) -- and its 8 warps work independently: a warp takes a block of 16 rows from a device queue, loads those
+// rows of B straight into registers in A-fragment layout (16 x K doubles = 72 per lane at K = 144), and runs the
+// whole K loop out of registers and the resident matrix, 48 output columns at a time.  No operand ever waits on
+// another warp: there is no barrier in the steady state, and a row's E (or V) is complete inside one warp, so no
+// partial row-dots are left for later.  CTAs that run out of blocks of their matrix switch to the other one.
+constexpr int kQrWarps = 8;
+constexpr int kQrNB = 6;  // n8 blocks (48 columns) per pass: 24 accumulator doubles per lane
+
+struct QrArgs {
+    const double* Bh;
+    double* W;
+    double* part;  // [2][max_ntn][chunk_cap]; these groups have one tile along N
+    const int* group_start;
+    const double* beta;
+    const double* sigma;  // may be null
+    int g, row0, nrows, ld, n_mat, chunk_cap, max_ntn;
+    int* counter;  // [2]: next 16-row block of the beta / Sigma queue (zeroed before the launch)
+};
+
+__device__ __forceinline__ void qr_mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void qr_mbar_expect(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes));
+}
+__device__ __forceinline__ void qr_bulk_row(void* smem_dst, const void* gmem_src, unsigned bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void qr_mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+template <int K16>  // K = 16 K16
+__global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
+    constexpr int K = 16 * K16;
+    constexpr int KS = K / 4;      // k4 steps
+    constexpr int MS = K + 4;      // padded row of the resident matrix (= 4 mod 16: conflict-free operand loads)
+    constexpr int NBT = K / 8;     // n8 blocks of the full width
+    constexpr int NP = (NBT + kQrNB - 1) / kQrNB;  // passes over the columns
+    extern __shared__ __align__(16) double smem[];
+    double* Ms = smem;  // [K][MS]: row n holds M[n][0..K) = column n of the symmetric matrix
+    __shared__ uint64_t bar;
+    __shared__ int s_switch;
+
+    const int gs = max(a.group_start[a.g], a.row0);
+    const int ge = min(a.group_start[a.g + 1], a.row0 + a.nrows);
+    const int n_rows = ge - gs;
+    if (n_rows <= 0) return;
+    const int lrow0 = gs - a.row0;
+    const int n_items = (n_rows + 15) / 16;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int g8 = lane >> 2, t4 = lane & 3;
+
+    // which matrix this CTA starts with: Sigma items cost ~0.56 of a beta item (upper triangle only)
+    int mat = (a.n_mat == 2 && ((blockIdx.x * 5) % 14) < 5) ? 1 : 0;
+    unsigned phase = 0;
+    if (tid == 0) {
+        qr_mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+    }
+    __syncthreads();
+    for (int round = 0; round < 2; round++) {
+        // ---- fetch the matrix: K bulk copies of one row each into the padded rows
+        if (tid == 0) {
+            asm volatile("fence.proxy.async.shared::cta;\n" ::);  // earlier generic-proxy reads of Ms are done (syncthreads)
+            const double* M = mat == 0 ? a.beta : a.sigma;
+            qr_mbar_expect(&bar, (unsigned)(K * K * sizeof(double)));
+            for (int n = 0; n < K; n++) qr_bulk_row(Ms + n * MS, M + (size_t)n * K, (unsigned)(K * sizeof(double)), &bar);
+        }
+        qr_mbar_wait(&bar, phase);
+        phase ^= 1u;
+
+        int* queue = a.counter + mat;
+        double* part = a.part + (size_t)mat * a.max_ntn * a.chunk_cap;
+        // the queue is read one block ahead: the atomic's round trip hides under the current block's K loop
+        int next = 0;
+        if (lane == 0) next = atomicAdd(queue, 1);
+        for (;;) {
+            const int item = __shfl_sync(kFull, next, 0);
+            if (item >= n_items) break;
+            if (lane == 0) next = atomicAdd(queue, 1);
+            const int r_lo = item * 16 + g8;  // rows of this lane inside the group: r_lo and r_lo + 8
+            const bool ok0 = r_lo < n_rows, ok1 = r_lo + 8 < n_rows;
+            const double* b0 = a.Bh + (size_t)(lrow0 + (ok0 ? r_lo : 0)) * a.ld;
+            const double* b1 = a.Bh + (size_t)(lrow0 + (ok1 ? r_lo + 8 : 0)) * a.ld;
+            // the 16 rows of B in A-fragment layout: lane (g8, t4) holds B[row g8 (+8)][4 ks + t4]
+            double af[2][KS];
+#pragma unroll
+            for (int ks = 0; ks < KS; ks++) {
+                af[0][ks] = ok0 ? __ldg(b0 + 4 * ks + t4) : 0.0;
+                af[1][ks] = ok1 ? __ldg(b1 + 4 * ks + t4) : 0.0;
+            }
+            double dot0 = 0.0, dot1 = 0.0;
+            for (int p = 0; p < NP; p++) {
+                double acc[2][kQrNB][2];
+#pragma unroll
+                for (int nb = 0; nb < kQrNB; nb++) { acc[0][nb][0] = acc[0][nb][1] = acc[1][nb][0] = acc[1][nb][1] = 0.0; }
+                const int nb0 = p * kQrNB;  // first n8 block of the pass
+                const double* ms = Ms + (size_t)(nb0 * 8 + g8) * MS + t4;
+                if (mat == 0) {
+#pragma unroll
+                    for (int ks = 0; ks < KS; ks++) {
+#pragma unroll
+                        for (int nb = 0; nb < kQrNB; nb++) {
+                            if (NBT % kQrNB == 0 || nb0 + nb < NBT) {
+                                const double b = ms[nb * 8 * MS + 4 * ks];
+                                dmma884(acc[0][nb][0], acc[0][nb][1], af[0][ks], b);
+                                dmma884(acc[1][nb][0], acc[1][nb][1], af[1][ks], b);
+                            }
+                        }
+                    }
+                } else {
+                    // symmetric matrix: only the 16 x 16 super-blocks with column block >= k block, the strictly upper
+                    // ones with a doubled operand (decided per pair of n8 blocks = one super-block: warp-uniform)
+#pragma unroll
+                    for (int ks = 0; ks < KS; ks++) {
+                        const int sk = ks >> 2;
+                        const double d0 = 2.0 * af[0][ks], d1 = 2.0 * af[1][ks];
+#pragma unroll
+                        for (int nb = 0; nb < kQrNB; nb += 2) {
+                            const int sn = (nb0 + nb) >> 1;  // super-block of this pair of column blocks
+                            if (sn >= sk && (NBT % kQrNB == 0 || nb0 + nb < NBT)) {
+                                const double x0 = sn > sk ? d0 : af[0][ks], x1 = sn > sk ? d1 : af[1][ks];
+#pragma unroll
+                                for (int e = 0; e < 2; e++) {
+                                    const double b = ms[(nb + e) * 8 * MS + 4 * ks];
+                                    dmma884(acc[0][nb + e][0], acc[0][nb + e][1], x0, b);
+                                    dmma884(acc[1][nb + e][0], acc[1][nb + e][1], x1, b);
+                                }
+                            }
+                        }
+                    }
+                }
+                // ---- epilogue of the pass: W store (beta) and the row-dot with B of the same columns.  B[row][c] of the
+                // accumulator's columns c = 8 nb + 2 t4 + e sits in the A fragments of the same quad: lane t4' = c & 3 =
+                // 2 (t4 & 1) + e, register ks = c >> 2 = 2 nb + (t4 >> 1) -- fetched by shuffles, not from memory
+                const int src0 = (lane & ~3) | (2 * (t4 & 1));
+                const bool hi = (t4 >> 1) != 0;
+#pragma unroll
+                for (int nb = 0; nb < kQrNB; nb++) {
+                    if (NBT % kQrNB == 0 || nb0 + nb < NBT) {
+                        // af index must be a compile-time constant: the pass index p is not, so select over the passes
+                        double bq[2][2];  // [row half][e]
+#pragma unroll
+                        for (int h = 0; h < 2; h++) {
+                            double lo_v = 0.0, hi_v = 0.0;
+#pragma unroll
+                            for (int pp = 0; pp < NP; pp++) {
+                                if (pp == p) {
+                                    const int kk = 2 * (pp * kQrNB + nb);
+                                    if (kk + 1 < KS) { lo_v = af[h][kk]; hi_v = af[h][kk + 1]; }
+                                }
+                            }
+#pragma unroll
+                            for (int e = 0; e < 2; e++) {
+                                const double x = __shfl_sync(kFull, lo_v, src0 + e);
+                                const double y = __shfl_sync(kFull, hi_v, src0 + e);
+                                bq[h][e] = hi ? y : x;
+                            }
+                        }
+                        const int c = (nb0 + nb) * 8 + 2 * t4;
+                        dot0 = fma(acc[0][nb][0], bq[0][0], dot0);
+                        dot0 = fma(acc[0][nb][1], bq[0][1], dot0);
+                        dot1 = fma(acc[1][nb][0], bq[1][0], dot1);
+                        dot1 = fma(acc[1][nb][1], bq[1][1], dot1);
+                        if (mat == 0) {
+                            if (ok0) *reinterpret_cast<double2*>(a.W + (size_t)(lrow0 + r_lo) * a.ld + c) = make_double2(acc[0][nb][0], acc[0][nb][1]);
+                            if (ok1) *reinterpret_cast<double2*>(a.W + (size_t)(lrow0 + r_lo + 8) * a.ld + c) = make_double2(acc[1][nb][0], acc[1][nb][1]);
+                        }
+                    }
+                }
+            }
+            dot0 += __shfl_xor_sync(kFull, dot0, 1);
+            dot0 += __shfl_xor_sync(kFull, dot0, 2);
+            dot1 += __shfl_xor_sync(kFull, dot1, 1);
+            dot1 += __shfl_xor_sync(kFull, dot1, 2);
+            if (t4 == 0) {
+                if (ok0) part[lrow0 + r_lo] = dot0;
+                if (ok1) part[lrow0 + r_lo + 8] = dot1;
+            }
+        }
+        // ---- this matrix's queue is empty: help with the other one if it still has blocks
+        if (a.n_mat < 2) break;
+        __syncthreads();  // every warp is done with the resident matrix
+        if (tid == 0) s_switch = (atomicAdd(a.counter + (mat ^ 1), 0) < n_items) ? 1 : 0;
+        __syncthreads();
+        if (!s_switch) break;
+        mat ^= 1;
+    }
+}
+
+template <int K16>
+static void launch_qform_res(Launcher& L, const QrArgs& a, int sm_count) {
+    constexpr int K = 16 * K16;
+    const size_t smem = sizeof(double) * (size_t)K * (K + 4);
+    L.ensure_smem(k_qform_res<K16>, smem);
+    const long long items = ((long long)a.nrows + 15) / 16;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(sm_count, (items + kQrWarps - 1) / kQrWarps));
+    L.launch(k_qform_res<K16>, dim3(grid), dim3(kQrWarps * 32), smem, a);
+}
+
 void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_groups, int row0, int nrows, int ld,
                int chunk_cap, bool want_variance, int sm_count) {
     if (nrows <= 0) return;
     int max_ntn = 0;
     for (int g = 0; g < n_groups; g++) max_ntn = groups[g].ntn > max_ntn ? groups[g].ntn : max_ntn;
-    L.memset(ws.qf_counter, 0, sizeof(int) * kMaxGroups);
+    L.memset(ws.qf_counter, 0, sizeof(int) * 3 * kMaxGroups);  // tile queues; [kMaxGroups + 2 g]: the two block queues of k_qform_res
     for (int g = 0; g < n_groups; g++) {
         const GroupDesc& gd = groups[g];
         if (gd.K == 0 || gd.beta == nullptr) continue;
@@ -299,6 +519,25 @@ void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_
         a.n_mat = (want_variance && gd.sigma) ? 2 : 1;
         a.chunk_cap = chunk_cap; a.max_ntn = max_ntn;
         a.counter = ws.qf_counter + g;
+        if (gd.K <= 144) {  // matrix resident in shared memory, warps independent
+            QrArgs r;
+            r.Bh = ws.Bh; r.W = ws.W; r.part = ws.part; r.group_start = ws.group_start;
+            r.beta = gd.beta; r.sigma = gd.sigma;
+            r.g = g; r.row0 = row0; r.nrows = nrows; r.ld = ld; r.n_mat = a.n_mat;
+            r.chunk_cap = chunk_cap; r.max_ntn = max_ntn;
+            r.counter = ws.qf_counter + kMaxGroups + 2 * g;
+            switch (gd.K / 16) {
+#define FLARE_CASE(KV)                            \
+    case KV:                                      \
+        launch_qform_res<KV>(L, r, sm_count);     \
+        break;
+                FLARE_CASE(1) FLARE_CASE(2) FLARE_CASE(3) FLARE_CASE(4) FLARE_CASE(5) FLARE_CASE(6) FLARE_CASE(7)
+                FLARE_CASE(8) FLARE_CASE(9)
+#undef FLARE_CASE
+                default: break;
+            }
+            continue;
+        }
         switch (gd.nb) {
 #define FLARE_CASE(NBV)                                                   \
     case NBV:                                                             \
