@@ -16,6 +16,7 @@
 // of a row are summed in fixed order by the back-propagation kernel (deterministic, atomics-free).
 // The rows hold the UNNORMALISED B; the 1/||B||^2 factor is applied by the back-propagation kernel.
 #include <algorithm>
+#include <type_traits>
 
 #include "kernels.cuh"
 
@@ -334,13 +335,14 @@ __device__ __forceinline__ void qr_mbar_wait(uint64_t* bar, unsigned parity) {
         : "memory");
 }
 
-template <int K16>  // K = 16 K16
-__global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
+template <int K16, int H>  // K = 16 K16; a warp's block is 8 H rows (H = 1: 16 warps per CTA, H = 2: 8 warps)
+__global__ void __launch_bounds__(kQrWarps * 32 * (3 - H), 1) k_qform_res(QrArgs a) {
     constexpr int K = 16 * K16;
     constexpr int KS = K / 4;      // k4 steps
     constexpr int MS = K + 4;      // padded row of the resident matrix (= 4 mod 16: conflict-free operand loads)
     constexpr int NBT = K / 8;     // n8 blocks of the full width
     constexpr int NP = (NBT + kQrNB - 1) / kQrNB;  // passes over the columns
+    constexpr int RB = 8 * H;      // rows per block
     extern __shared__ __align__(16) double smem[];
     double* Ms = smem;  // [K][MS]: row n holds M[n][0..K) = column n of the symmetric matrix
     __shared__ uint64_t bar;
@@ -351,7 +353,7 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
     const int n_rows = ge - gs;
     if (n_rows <= 0) return;
     const int lrow0 = gs - a.row0;
-    const int n_items = (n_rows + 15) / 16;
+    const int n_items = (n_rows + RB - 1) / RB;
     const int tid = threadIdx.x, lane = tid & 31;
     const int g8 = lane >> 2, t4 = lane & 3;
 
@@ -383,22 +385,29 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
             const int item = __shfl_sync(kFull, next, 0);
             if (item >= n_items) break;
             if (lane == 0) next = atomicAdd(queue, 1);
-            const int r_lo = item * 16 + g8;  // rows of this lane inside the group: r_lo and r_lo + 8
-            const bool ok0 = r_lo < n_rows, ok1 = r_lo + 8 < n_rows;
-            const double* b0 = a.Bh + (size_t)(lrow0 + (ok0 ? r_lo : 0)) * a.ld;
-            const double* b1 = a.Bh + (size_t)(lrow0 + (ok1 ? r_lo + 8 : 0)) * a.ld;
-            // the 16 rows of B in A-fragment layout: lane (g8, t4) holds B[row g8 (+8)][4 ks + t4]
-            double af[2][KS];
+            const int r_lo = item * RB + g8;  // rows of this lane inside the group: r_lo (and r_lo + 8)
+            bool ok[H];
+            const double* brow[H];
 #pragma unroll
-            for (int ks = 0; ks < KS; ks++) {
-                af[0][ks] = ok0 ? __ldg(b0 + 4 * ks + t4) : 0.0;
-                af[1][ks] = ok1 ? __ldg(b1 + 4 * ks + t4) : 0.0;
+            for (int h = 0; h < H; h++) {
+                ok[h] = r_lo + 8 * h < n_rows;
+                brow[h] = a.Bh + (size_t)(lrow0 + (ok[h] ? r_lo + 8 * h : 0)) * a.ld;
             }
-            double dot0 = 0.0, dot1 = 0.0;
-            for (int p = 0; p < NP; p++) {
-                double acc[2][kQrNB][2];
+            // the rows of B in A-fragment layout: lane (g8, t4) holds B[row g8 (+8)][4 ks + t4]
+            double af[H][KS];
 #pragma unroll
-                for (int nb = 0; nb < kQrNB; nb++) { acc[0][nb][0] = acc[0][nb][1] = acc[1][nb][0] = acc[1][nb][1] = 0.0; }
+            for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+                for (int h = 0; h < H; h++) af[h][ks] = ok[h] ? __ldg(brow[h] + 4 * ks + t4) : 0.0;
+            double dot[H];
+#pragma unroll
+            for (int h = 0; h < H; h++) dot[h] = 0.0;
+            for (int p = 0; p < NP; p++) {
+                double acc[H][kQrNB][2];
+#pragma unroll
+                for (int h = 0; h < H; h++)
+#pragma unroll
+                    for (int nb = 0; nb < kQrNB; nb++) { acc[h][nb][0] = 0.0; acc[h][nb][1] = 0.0; }
                 const int nb0 = p * kQrNB;  // first n8 block of the pass
                 const double* ms = Ms + (size_t)(nb0 * 8 + g8) * MS + t4;
                 if (mat == 0) {
@@ -408,31 +417,48 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
                         for (int nb = 0; nb < kQrNB; nb++) {
                             if (NBT % kQrNB == 0 || nb0 + nb < NBT) {
                                 const double b = ms[nb * 8 * MS + 4 * ks];
-                                dmma884(acc[0][nb][0], acc[0][nb][1], af[0][ks], b);
-                                dmma884(acc[1][nb][0], acc[1][nb][1], af[1][ks], b);
+#pragma unroll
+                                for (int h = 0; h < H; h++) dmma884(acc[h][nb][0], acc[h][nb][1], af[h][ks], b);
                             }
                         }
                     }
                 } else {
                     // symmetric matrix: only the 16 x 16 super-blocks with column block >= k block, the strictly upper
-                    // ones with a doubled operand (decided per pair of n8 blocks = one super-block: warp-uniform)
+                    // ones with a doubled operand.  One warp-uniform decision per k super-block picks a straight-line
+                    // block of DMMAs (a per-DMMA condition ends up predicated, and a predicated-off DMMA still costs
+                    // its pipe slot): `first` = first super-block of the pass that is needed, `diag` = it is the diagonal one.
+                    const int sb0 = nb0 >> 1;  // first 16-column super-block of the pass
 #pragma unroll
-                    for (int ks = 0; ks < KS; ks++) {
-                        const int sk = ks >> 2;
-                        const double d0 = 2.0 * af[0][ks], d1 = 2.0 * af[1][ks];
+                    for (int sk = 0; sk < K16; sk++) {
+                        auto blk = [&](auto first_c, auto diag_c) {
+                            constexpr int FIRST = decltype(first_c)::value;
+                            constexpr bool DIAG = decltype(diag_c)::value;
 #pragma unroll
-                        for (int nb = 0; nb < kQrNB; nb += 2) {
-                            const int sn = (nb0 + nb) >> 1;  // super-block of this pair of column blocks
-                            if (sn >= sk && (NBT % kQrNB == 0 || nb0 + nb < NBT)) {
-                                const double x0 = sn > sk ? d0 : af[0][ks], x1 = sn > sk ? d1 : af[1][ks];
+                            for (int k4 = 0; k4 < 4; k4++) {
+                                const int ks = 4 * sk + k4;
 #pragma unroll
-                                for (int e = 0; e < 2; e++) {
-                                    const double b = ms[(nb + e) * 8 * MS + 4 * ks];
-                                    dmma884(acc[0][nb + e][0], acc[0][nb + e][1], x0, b);
-                                    dmma884(acc[1][nb + e][0], acc[1][nb + e][1], x1, b);
+                                for (int sb = FIRST; sb < kQrNB / 2; sb++) {
+                                    if (NBT % kQrNB == 0 || nb0 + 2 * sb < NBT) {
+#pragma unroll
+                                        for (int e = 0; e < 2; e++) {
+                                            const double b = ms[(2 * sb + e) * 8 * MS + 4 * ks];
+#pragma unroll
+                                            for (int h = 0; h < H; h++)
+                                                dmma884(acc[h][2 * sb + e][0], acc[h][2 * sb + e][1],
+                                                        (DIAG && sb == FIRST) ? af[h][ks] : 2.0 * af[h][ks], b);
+                                        }
+                                    }
                                 }
                             }
-                        }
+                        };
+                        using I0 = std::integral_constant<int, 0>;
+                        using I1 = std::integral_constant<int, 1>;
+                        using I2 = std::integral_constant<int, 2>;
+                        const int d = sk - sb0;  // which super-block of the pass is the diagonal one
+                        if (d < 0) blk(I0{}, std::false_type{});
+                        else if (d == 0) blk(I0{}, std::true_type{});
+                        else if (d == 1) blk(I1{}, std::true_type{});
+                        else if (d == 2) blk(I2{}, std::true_type{});
                     }
                 }
                 // ---- epilogue of the pass: W store (beta) and the row-dot with B of the same columns.  B[row][c] of the
@@ -443,10 +469,10 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
 #pragma unroll
                 for (int nb = 0; nb < kQrNB; nb++) {
                     if (NBT % kQrNB == 0 || nb0 + nb < NBT) {
-                        // af index must be a compile-time constant: the pass index p is not, so select over the passes
-                        double bq[2][2];  // [row half][e]
+                        const int c = (nb0 + nb) * 8 + 2 * t4;
 #pragma unroll
-                        for (int h = 0; h < 2; h++) {
+                        for (int h = 0; h < H; h++) {
+                            // the af index must be a compile-time constant and the pass index p is not: select over the passes
                             double lo_v = 0.0, hi_v = 0.0;
 #pragma unroll
                             for (int pp = 0; pp < NP; pp++) {
@@ -455,32 +481,21 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
                                     if (kk + 1 < KS) { lo_v = af[h][kk]; hi_v = af[h][kk + 1]; }
                                 }
                             }
-#pragma unroll
-                            for (int e = 0; e < 2; e++) {
-                                const double x = __shfl_sync(kFull, lo_v, src0 + e);
-                                const double y = __shfl_sync(kFull, hi_v, src0 + e);
-                                bq[h][e] = hi ? y : x;
-                            }
-                        }
-                        const int c = (nb0 + nb) * 8 + 2 * t4;
-                        dot0 = fma(acc[0][nb][0], bq[0][0], dot0);
-                        dot0 = fma(acc[0][nb][1], bq[0][1], dot0);
-                        dot1 = fma(acc[1][nb][0], bq[1][0], dot1);
-                        dot1 = fma(acc[1][nb][1], bq[1][1], dot1);
-                        if (mat == 0) {
-                            if (ok0) *reinterpret_cast<double2*>(a.W + (size_t)(lrow0 + r_lo) * a.ld + c) = make_double2(acc[0][nb][0], acc[0][nb][1]);
-                            if (ok1) *reinterpret_cast<double2*>(a.W + (size_t)(lrow0 + r_lo + 8) * a.ld + c) = make_double2(acc[1][nb][0], acc[1][nb][1]);
+                            const double x0 = __shfl_sync(kFull, lo_v, src0), y0 = __shfl_sync(kFull, hi_v, src0);
+                            const double x1 = __shfl_sync(kFull, lo_v, src0 + 1), y1 = __shfl_sync(kFull, hi_v, src0 + 1);
+                            dot[h] = fma(acc[h][nb][0], hi ? y0 : x0, dot[h]);
+                            dot[h] = fma(acc[h][nb][1], hi ? y1 : x1, dot[h]);
+                            if (mat == 0 && ok[h])
+                                *reinterpret_cast<double2*>(a.W + (size_t)(lrow0 + r_lo + 8 * h) * a.ld + c) = make_double2(acc[h][nb][0], acc[h][nb][1]);
                         }
                     }
                 }
             }
-            dot0 += __shfl_xor_sync(kFull, dot0, 1);
-            dot0 += __shfl_xor_sync(kFull, dot0, 2);
-            dot1 += __shfl_xor_sync(kFull, dot1, 1);
-            dot1 += __shfl_xor_sync(kFull, dot1, 2);
-            if (t4 == 0) {
-                if (ok0) part[lrow0 + r_lo] = dot0;
-                if (ok1) part[lrow0 + r_lo + 8] = dot1;
+#pragma unroll
+            for (int h = 0; h < H; h++) {
+                dot[h] += __shfl_xor_sync(kFull, dot[h], 1);
+                dot[h] += __shfl_xor_sync(kFull, dot[h], 2);
+                if (t4 == 0 && ok[h]) part[lrow0 + r_lo + 8 * h] = dot[h];
             }
         }
         // ---- this matrix's queue is empty: help with the other one if it still has blocks
@@ -493,14 +508,17 @@ __global__ void __launch_bounds__(kQrWarps * 32, 1) k_qform_res(QrArgs a) {
     }
 }
 
+constexpr int kQrH = 1;  // rows per warp block / 8
+
 template <int K16>
 static void launch_qform_res(Launcher& L, const QrArgs& a, int sm_count) {
     constexpr int K = 16 * K16;
+    constexpr int warps = kQrWarps * (3 - kQrH);
     const size_t smem = sizeof(double) * (size_t)K * (K + 4);
-    L.ensure_smem(k_qform_res<K16>, smem);
-    const long long items = ((long long)a.nrows + 15) / 16;
-    const int grid = (int)std::max<long long>(1, std::min<long long>(sm_count, (items + kQrWarps - 1) / kQrWarps));
-    L.launch(k_qform_res<K16>, dim3(grid), dim3(kQrWarps * 32), smem, a);
+    L.ensure_smem(k_qform_res<K16, kQrH>, smem);
+    const long long items = ((long long)a.nrows + 8 * kQrH - 1) / (8 * kQrH);
+    const int grid = (int)std::max<long long>(1, std::min<long long>(sm_count, (items + warps - 1) / warps));
+    L.launch(k_qform_res<K16, kQrH>, dim3(grid), dim3(warps * 32), smem, a);
 }
 
 void run_qform(Launcher& L, const Workspace& ws, const GroupDesc* groups, int n_groups, int row0, int nrows, int ld,
