@@ -87,21 +87,39 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     const int T = __shfl_sync(kFull, my_end, kDescTA - 1);
     __syncwarp();
 
+    // the loads of a pass are issued ahead of their use: the neighbour INDEX of pass q+2 and the two ATOMS of pass q+1
+    // are requested during pass q (the kernel is otherwise stalled on these dependent, scattered 32-byte reads)
+    auto locate = [&](int p, int& k, int& s) {
+        int ai = 0;
+#pragma unroll
+        for (int i = 0; i < kDescTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
+        k = __shfl_sync(kFull, my_k, ai);
+        s = p - __shfl_sync(kFull, my_start, ai);
+    };
+    int k_n, s_n, j_n = 0, k_nn, s_nn, j_nn = 0;
+    locate(lane, k_n, s_n);
+    if (lane < T) j_n = nbr_idx[(size_t)k_n * mmax + s_n];
+    locate(lane + 32, k_nn, s_nn);
+    if (lane + 32 < T) j_nn = nbr_idx[(size_t)k_nn * mmax + s_nn];
+    AtomS me_n = load_atom(atoms + k_n), o_n = load_atom(atoms + j_n);
+
     int a = 0;
     for (int p0 = 0;; p0 += 32) {
         // ---- 1. stage the basis of pairs [p0, p0+32)
         if (p0 < T) {
             const int p = p0 + lane;
-            int ai = 0;
-#pragma unroll
-            for (int i = 0; i < kDescTA - 1; i++) ai += (p >= __shfl_sync(kFull, my_end, i)) ? 1 : 0;
-            const int k = __shfl_sync(kFull, my_k, ai);
-            const int s = p - __shfl_sync(kFull, my_start, ai);
+            const AtomS me = me_n, o = o_n;
+            if (p0 + 32 < T) {  // uniform
+                k_n = k_nn; j_n = j_nn;
+                me_n = load_atom(atoms + k_n);
+                o_n = load_atom(atoms + j_n);
+                if (p0 + 64 < T) {  // uniform
+                    locate(p + 64, k_nn, s_nn);
+                    j_nn = (p + 64 < T) ? nbr_idx[(size_t)k_nn * mmax + s_nn] : 0;
+                }
+            }
             int sj = -1;
             if (p < T) {
-                const int j = nbr_idx[(size_t)k * mmax + s];
-                const AtomS me = load_atom(atoms + k);
-                const AtomS o = load_atom(atoms + j);
                 double dx, dy, dz;
                 displacement(g, me, o, dx, dy, dz);
                 const double r2 = dx * dx + dy * dy + dz * dz;
