@@ -480,64 +480,67 @@ __global__ void k_copy_ref(int n, const AtomS* __restrict__ atoms, AtomS* __rest
     if (k == 0) *n_rebuilds += 1;  // statistics (FLARE_OPT_SKIN_REBUILDS)
 }
 
-// A warp takes kFilterAtoms consecutive atoms at a time: lane s tests candidate s of each atom's skin row with the exact
-// predicate; the index and atom loads of all of them are issued before the first test (the kernel is bound by the latency
-// of the scattered 32-byte atom reads), hits are compacted into nbr_idx by ballot.
-constexpr int kFilterAtoms = 1;  // measured: 1 atom per warp pass 0.36 ms, 4 atoms 0.47 ms on C3
+// A warp takes kFilterAtoms consecutive atoms, 8 lanes each: a lane tests candidates l8, l8 + 8, ... of its atom's skin row
+// with the exact predicate, four at a time, their index and atom loads issued before the first test (the kernel is bound
+// by the latency of the scattered 32-byte atom reads: with ~22 candidates per row, 8 lanes per atom keep the lanes full
+// and three to four reads per lane in flight); hits are compacted into nbr_idx, in candidate order, by ballot.
+constexpr int kFilterAtoms = 4;  // atoms per warp: 8 lanes each
 
 __global__ void __launch_bounds__(kNbrWarps * 32)
 k_filter(Grid g, Basis bs, int n, int mmax, int smax, const AtomS* __restrict__ atoms, const int* __restrict__ skin_cnt,
          const int* __restrict__ skin_idx, int* __restrict__ nbr_cnt, int* __restrict__ nbr_idx,
          unsigned char* __restrict__ nmask, unsigned long long* __restrict__ hitmask, int* __restrict__ flags) {
+    constexpr int LPA = 32 / kFilterAtoms;  // lanes per atom
+    constexpr int UN = 4;                   // candidates per lane whose loads fly together (UN * LPA = 32 per chunk)
     const int lane = threadIdx.x & 31;
-    const int k0 = (blockIdx.x * kNbrWarps + (threadIdx.x >> 5)) * kFilterAtoms;
-    if (k0 >= n) return;
-    int sc[kFilterAtoms], cnt[kFilterAtoms];
-    unsigned mask[kFilterAtoms];
-    unsigned long long hm[kFilterAtoms];
-    AtomS me[kFilterAtoms];
-    int scmax = 0;
+    const int sub = lane / LPA, l8 = lane % LPA;
+    const int k = (blockIdx.x * kNbrWarps + (threadIdx.x >> 5)) * kFilterAtoms + sub;
+    const bool live = k < n;
+    const int sc = live ? skin_cnt[k] : 0;
+    const AtomS me = load_atom(atoms + (live ? k : 0));
+    const unsigned grp = ((1u << LPA) - 1u) << (sub * LPA);  // ballot bits of this atom's lanes
+    int cnt = 0;
+    unsigned mask = 0;
+    unsigned long long hm = 0;
+    int scmax = sc;
 #pragma unroll
-    for (int a = 0; a < kFilterAtoms; a++) {
-        const int k = min(k0 + a, n - 1);
-        sc[a] = (k0 + a < n) ? skin_cnt[k] : 0;
-        me[a] = load_atom(atoms + k);
-        cnt[a] = 0; mask[a] = 0; hm[a] = 0;
-        scmax = max(scmax, sc[a]);
-    }
-    for (int base = 0; base < scmax; base += 32) {  // at most 2 passes (rows hold <= 64 candidates)
-        const int s = base + lane;
-        int j[kFilterAtoms];
-        AtomS o[kFilterAtoms];
+    for (int o = 16; o > 0; o >>= 1) scmax = max(scmax, __shfl_xor_sync(kFull, scmax, o));
+    for (int base = 0; base < scmax; base += UN * LPA) {  // at most 2 chunks (rows hold <= 64 candidates)
+        int j[UN];
+        AtomS o[UN];
 #pragma unroll
-        for (int a = 0; a < kFilterAtoms; a++) j[a] = (s < sc[a]) ? skin_idx[(size_t)(k0 + a) * smax + s] : 0;
+        for (int u = 0; u < UN; u++) {
+            const int s = base + u * LPA + l8;
+            j[u] = (s < sc) ? skin_idx[(size_t)k * smax + s] : 0;
+        }
 #pragma unroll
-        for (int a = 0; a < kFilterAtoms; a++) o[a] = load_atom(atoms + j[a]);
+        for (int u = 0; u < UN; u++) o[u] = load_atom(atoms + j[u]);
 #pragma unroll
-        for (int a = 0; a < kFilterAtoms; a++) {
+        for (int u = 0; u < UN; u++) {  // candidate order s = base + u LPA + l8: ascending in (u, lane), as the list expects
+            const int s = base + u * LPA + l8;
             double dx, dy, dz;
-            displacement(g, me[a], o[a], dx, dy, dz);
-            const bool hit = (s < sc[a]) && dist2_canonical(dx, dy, dz) < bs.rc2[me[a].type * bs.S + o[a].type];  // strict (R6)
-            const unsigned b = __ballot_sync(kFull, hit);
+            displacement(g, me, o[u], dx, dy, dz);
+            const bool hit = (s < sc) && dist2_canonical(dx, dy, dz) < bs.rc2[me.type * bs.S + o[u].type];  // strict (R6)
+            const unsigned b = __ballot_sync(kFull, hit) & grp;
             if (hit) {
-                const int slot = cnt[a] + __popc(b & ((1u << lane) - 1u));
-                if (slot < mmax) nbr_idx[(size_t)(k0 + a) * mmax + slot] = j[a];
-                mask[a] |= 1u << o[a].type;
+                const int slot = cnt + __popc(b & ((1u << lane) - 1u));
+                if (slot < mmax) nbr_idx[(size_t)k * mmax + slot] = j[u];
+                mask |= 1u << o[u].type;
+                hm |= 1ull << s;
             }
-            cnt[a] += __popc(b);
-            hm[a] |= (unsigned long long)b << base;
+            cnt += __popc(b);
         }
     }
 #pragma unroll
-    for (int a = 0; a < kFilterAtoms; a++) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mask[a] |= __shfl_xor_sync(kFull, mask[a], o);
-        if (lane == 0 && k0 + a < n) {
-            if (cnt[a] > mmax) { atomicOr(flags, kFlagNeighborOverflow); cnt[a] = mmax; }
-            nbr_cnt[k0 + a] = cnt[a];
-            nmask[k0 + a] = (unsigned char)mask[a];
-            hitmask[k0 + a] = hm[a];
-        }
+    for (int o = LPA / 2; o > 0; o >>= 1) {
+        mask |= __shfl_xor_sync(kFull, mask, o);
+        hm |= __shfl_xor_sync(kFull, hm, o);
+    }
+    if (l8 == 0 && live) {
+        if (cnt > mmax) { atomicOr(flags, kFlagNeighborOverflow); cnt = mmax; }
+        nbr_cnt[k] = cnt;
+        nmask[k] = (unsigned char)mask;
+        hitmask[k] = hm;
     }
 }
 
