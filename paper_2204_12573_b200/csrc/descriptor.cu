@@ -16,6 +16,8 @@
 //      the tensor pipe, stored straight from the accumulator fragments (the L values of one (cnu1,cnu2)
 //      pair are contiguous), and ||B||.  B is stored UNNORMALISED: d^ = B/||B|| is applied by the
 //      consumers (E = B^T beta B / ||B||^2), which saves a second pass over the row.
+#include <algorithm>
+
 #include "kernels.cuh"
 
 namespace flare {
@@ -58,8 +60,9 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     // rows of this group inside the chunk
     const int gs_ = max(group_start[gr.g], gr.row0);
     const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
-    const int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA;
-    if (r0 >= ge_ - gs_) return;  // warps are independent: only __syncwarp below
+    // the grid is capped (a launch for a group with few or no rows costs next to nothing): a warp strides over its blocks
+    for (int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA; r0 < ge_ - gs_; r0 += gridDim.x * kDescWarps * kDescTA) {
+    // warps are independent: only __syncwarp below
     const int na = min(kDescTA, ge_ - gs_ - r0);
     const int lrow0 = gs_ - gr.row0 + r0;  // chunk-local row of the warp's first atom
     const int g8 = lane >> 2, t4 = lane & 3;
@@ -238,6 +241,8 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
         __syncwarp();
         if (a >= na) break;
     }
+    __syncwarp();
+    }  // blocks of this warp
 }
 
 template <int LMAX, int NMAXP>
@@ -248,7 +253,8 @@ static void launch_descriptor(Launcher& L, const Grid& g, const Basis& bs, const
     const size_t smem = sizeof(double) * kDescWarps * (size_t)SM::warp_doubles(Nc8);
     L.ensure_smem(k_descriptor<LMAX, NMAXP>, smem);
     const int per_cta = kDescWarps * kDescTA;
-    L.launch(k_descriptor<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(kDescWarps * 32), smem, g, bs, yn,
+    const int grid = std::min((gr.nrows + per_cta - 1) / per_cta, 148 * 32);
+    L.launch(k_descriptor<LMAX, NMAXP>, dim3(grid), dim3(kDescWarps * 32), smem, g, bs, yn,
              gr, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const int*)ws.group_start, write_A ? ws.A : (double*)nullptr, bh_out, ld,
              nrm_out);

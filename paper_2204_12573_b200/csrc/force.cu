@@ -11,6 +11,8 @@
 // f_kj is stored once per ordered pair.  k_gather then forms, with the reverse-pair index,
 //   F_k = sum_j ( f_kj - f_jk )
 // reading each pair force exactly twice and writing each atom's force exactly once.
+#include <algorithm>
+
 #include "kernels.cuh"
 
 namespace flare {
@@ -91,8 +93,10 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gs_ = max(group_start[gr.g], gr.row0);
     const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
-    const int r0 = (blockIdx.x * (blockDim.x >> 5) + warp) * ta;  // 1..kBpWarps warps per CTA (shared-memory budget)
-    if (r0 >= ge_ - gs_) return;  // warps are independent: only __syncwarp below
+    // 1..kBpWarps warps per CTA (shared-memory budget); the grid is capped (a launch for a group with few or no rows
+    // costs next to nothing): a warp strides over its blocks.  Warps are independent: only __syncwarp below.
+    const int wpc = blockDim.x >> 5;
+    for (int r0 = (blockIdx.x * wpc + warp) * ta; r0 < ge_ - gs_; r0 += gridDim.x * wpc * ta) {
     const int na = min(ta, ge_ - gs_ - r0);
     const int lrow0 = gs_ - gr.row0 + r0;
     const int g8 = lane >> 2, t4 = lane & 3;
@@ -290,6 +294,8 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
             pf[2] = srad * uz + (vz - uz * udv) * ir;
         }
     }
+    __syncwarp();
+    }  // blocks of this warp
 }
 
 template <int LMAX, int NMAXP>
@@ -320,7 +326,8 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
     }
     L.ensure_smem(k_backprop<LMAX, NMAXP>, smem);
     const int per_cta = warps * ta;
-    L.launch(k_backprop<LMAX, NMAXP>, dim3((gr.nrows + per_cta - 1) / per_cta), dim3(warps * 32), smem, g, bs, yn, gr,
+    const int grid = std::min((gr.nrows + per_cta - 1) / per_cta, 148 * 32);
+    L.launch(k_backprop<LMAX, NMAXP>, dim3(grid), dim3(warps * 32), smem, g, bs, yn, gr,
              ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const int*)ws.group_start, (const double*)ws.A, (const double*)ws.Bh,
              (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap, max_ntn,
