@@ -76,7 +76,7 @@ __device__ __forceinline__ void radial_fixed(int n_max, double r, double inv_rc,
 // G = dE/dA of each of its atoms (G on the tensor pipe), phase 2 walks over the concatenated neighbour
 // lists of those atoms, one pair per lane, so that the basis gradients run with nearly full lanes.
 template <int LMAX, int NMAXP>
-__global__ void __launch_bounds__(kBpWarps * 32)
+__global__ void __launch_bounds__(kBpWarps * 32, 4)
 k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restrict__ atoms,
            const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx, int mmax,
            const int* __restrict__ atom_of_row, const int* __restrict__ group_start, const double* __restrict__ A_in,
@@ -213,9 +213,23 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
                 const int cq = in ? (lo * Nc - (lo * (lo - 1)) / 2 + (hi - lo)) * L : 0;
                 const double fac = (nu1 == nu2) ? 2.0 * two_inv2 : two_inv2;  // (1 + delta) of the diagonal pairs
                 const double* a2 = As + nu2 * AS + g8;
+                // the L values of W and B of this channel pair are contiguous: fetched with 16-byte loads (half the
+                // shared-memory instructions, and the 8-byte loads at stride L were 4-way bank conflicts)
+                double wv[L], bvv[L];
+                if constexpr (L % 2 == 0) {
+#pragma unroll
+                    for (int l = 0; l < L; l += 2) {
+                        const double2 w2 = *reinterpret_cast<const double2*>(Ws + cq + l);
+                        const double2 b2 = *reinterpret_cast<const double2*>(Bs + cq + l);
+                        wv[l] = w2.x; wv[l + 1] = w2.y; bvv[l] = b2.x; bvv[l + 1] = b2.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int l = 0; l < L; l++) { wv[l] = Ws[cq + l]; bvv[l] = Bs[cq + l]; }
+                }
 #pragma unroll
                 for (int l = 0; l < L; l++) {
-                    const double av = in ? fac * (Ws[cq + l] - E * Bs[cq + l]) : 0.0;  // c = dE/dB
+                    const double av = in ? fac * (wv[l] - E * bvv[l]) : 0.0;  // c = dE/dB
 #pragma unroll
                     for (int nb = 0; nb < NBL; nb++) {
                         if (nb * 8 < 2 * l + 1) {
@@ -226,7 +240,8 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
                 }
             }
             if (nu1 < Nc) {
-                const int s1 = nu1 / n_max, n1 = nu1 - s1 * n_max;
+                int s1 = 0, n1 = nu1;  // species block of the channel (no division: at most nsp - 1 subtractions)
+                while (n1 >= n_max) { n1 -= n_max; s1++; }
                 double* gt = Gta + (size_t)s1 * GB + n1;
 #pragma unroll
                 for (int l = 0; l < L; l++)
