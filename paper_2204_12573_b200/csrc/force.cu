@@ -105,13 +105,28 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     double* Gt = smem + (size_t)warp * SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);  // [ta][nsp][GB]
     double* rows = Gt + ta * gr.nsp * GB;  // [2][ A [Nc8][AS] | W [K] | B [K] ]
     const int row_doubles = Nc8 * AS + 2 * gr.K;
-    for (int c = lane; c < ta * gr.nsp * GB + 2 * row_doubles; c += 32) Gt[c] = 0.0;  // G^T (n >= n_max stays 0), A padding
-
+    // the first loads of the block are issued before anything else: the atom of each row, and (lane a for atom a) the
+    // first tile partials and ||B|| that phase 1 starts from
     int my_k = 0, my_cnt = 0;
+    double pE0 = 0.0, pV0 = 0.0, pnrm = 0.0;
     if (lane < na) {
         my_k = atom_of_row[gs_ + r0 + lane];
-        my_cnt = nbr_cnt[my_k];
+        if (gr.ntn > 0) {
+            pE0 = part[lrow0 + lane];
+            if (want_variance) pV0 = part[(size_t)max_ntn * chunk_cap + lrow0 + lane];
+        }
+        if (gr.P > 0) pnrm = nrm_in[lrow0 + lane];
     }
+    // what is read without having been written: G^T rows n >= n_max (B operand of the pair phase) and the A rows of the
+    // padding channels Nc .. Nc8 (multiplied by a zero dE/dB, but 0 x NaN would poison the accumulator)
+    if (n_max < NMAXP)
+        for (int c = lane; c < ta * gr.nsp * GB; c += 32) Gt[c] = 0.0;
+    if (Nc < Nc8)
+        for (int c = lane; c < 2 * (Nc8 - Nc) * AS; c += 32) {
+            const int buf = c / ((Nc8 - Nc) * AS);
+            rows[buf * row_doubles + Nc * AS + (c - buf * (Nc8 - Nc) * AS)] = 0.0;
+        }
+    if (lane < na) my_cnt = nbr_cnt[my_k];
     int my_end = my_cnt;
 #pragma unroll
     for (int o = 1; o < kBpMaxTA; o <<= 1) {
@@ -148,11 +163,11 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     double my_E = 0.0, my_inv2 = 0.0;
     if (lane < na) {
         const int lrow = lrow0 + lane;
-        double E = 0.0, V = 0.0;
-        for (int t = 0; t < gr.ntn; t++) E += part[(size_t)t * chunk_cap + lrow];
+        double E = pE0, V = pV0;
+        for (int t = 1; t < gr.ntn; t++) E += part[(size_t)t * chunk_cap + lrow];
         if (want_variance)
-            for (int t = 0; t < gr.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + lrow];
-        const double nrm = (gr.P > 0) ? nrm_in[lrow] : 0.0;
+            for (int t = 1; t < gr.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + lrow];
+        const double nrm = pnrm;
         my_inv2 = (nrm > 0.0) ? 1.0 / (nrm * nrm) : 0.0;  // no neighbours: E = V = 0 (R8)
         my_E = E * my_inv2;
         e_s[my_k] = my_E;
