@@ -60,11 +60,6 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     // rows of this group inside the chunk
     const int gs_ = max(group_start[gr.g], gr.row0);
     const int ge_ = min(group_start[gr.g + 1], gr.row0 + gr.nrows);
-    // the grid is capped (a launch for a group with few or no rows costs next to nothing): a warp strides over its blocks
-    for (int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA; r0 < ge_ - gs_; r0 += gridDim.x * kDescWarps * kDescTA) {
-    // warps are independent: only __syncwarp below
-    const int na = min(kDescTA, ge_ - gs_ - r0);
-    const int lrow0 = gs_ - gr.row0 + r0;  // chunk-local row of the warp's first atom
     const int g8 = lane >> 2, t4 = lane & 3;
     const int n_max = bs.n_max;
     const int Nc = gr.Nc, Nc8 = (Nc + 7) & ~7, nmb = Nc8 >> 3;
@@ -72,7 +67,15 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     double* ysm = gsm + NMAXP * kPS;                             // [YR][kPS]
     double* As = ysm + SM::YR * kPS;                             // [Nc8][AS]
     int* sjs = reinterpret_cast<int*>(As + Nc8 * AS);            // [32] compact species of the staged pairs
-    for (int c = lane; c < (NMAXP + SM::YR) * kPS + Nc8 * AS; c += 32) gsm[c] = 0.0;
+    // zeroed once per warp: the staged rows keep finite values from then on (idle lanes' columns are masked by a zero
+    // operand, which needs a finite partner), the Y padding rows stay zero, and A is re-zeroed after every atom
+    if ((blockIdx.x * kDescWarps + warp) * kDescTA < ge_ - gs_)
+        for (int c = lane; c < (NMAXP + SM::YR) * kPS + Nc8 * AS; c += 32) gsm[c] = 0.0;
+    // the grid is capped (a launch for a group with few or no rows costs next to nothing): a warp strides over its blocks
+    for (int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA; r0 < ge_ - gs_; r0 += gridDim.x * kDescWarps * kDescTA) {
+    // warps are independent: only __syncwarp below
+    const int na = min(kDescTA, ge_ - gs_ - r0);
+    const int lrow0 = gs_ - gr.row0 + r0;  // chunk-local row of the warp's first atom
 
     // per-lane atom bookkeeping (lanes 0..na-1), inclusive scan of the neighbour counts
     int my_k = 0, my_cnt = 0;
