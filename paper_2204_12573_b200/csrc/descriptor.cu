@@ -67,6 +67,7 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     double* ysm = gsm + NMAXP * kPS;                             // [YR][kPS]
     double* As = ysm + SM::YR * kPS;                             // [Nc8][AS]
     int* sjs = reinterpret_cast<int*>(As + Nc8 * AS);            // [32] compact species of the staged pairs
+    const bool one_species = gr.nsp == 1;
     // zeroed once per warp: the staged rows keep finite values from then on (idle lanes' columns are masked by a zero
     // operand, which needs a finite partner), the Y padding rows stay zero, and A is re-zeroed after every atom
     if ((blockIdx.x * kDescWarps + warp) * kDescTA < ge_ - gs_)
@@ -159,14 +160,19 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
                 // B-operand (row j = k0+t4, col lm = 8nb+g8), C (row cnu = 8mb+g8, cols lm = 8nb+2t4, +1).
                 for (int mb = 0; mb < nmb; mb++) {
                     const int cnu = mb * 8 + g8;
-                    const int s_nu = (cnu < Nc) ? cnu / n_max : -2;
-                    const double* grow = gsm + (cnu < Nc ? cnu - s_nu * n_max : 0) * kPS;
+                    int s_nu = -2, n_nu = 0;  // species block and radial index of the channel (no division)
+                    if (cnu < Nc) {
+                        s_nu = 0; n_nu = cnu;
+                        while (n_nu >= n_max) { n_nu -= n_max; s_nu++; }
+                    }
+                    const double* grow = gsm + n_nu * kPS;
                     double acc[NBY][2];
 #pragma unroll
                     for (int nb = 0; nb < NBY; nb++) { acc[nb][0] = 0.0; acc[nb][1] = 0.0; }
                     for (int k0 = s0 & ~3; k0 < s1; k0 += 4) {
                         const int j = k0 + t4;
-                        const bool on = (j >= s0) && (j < s1) && (sjs[j] == s_nu);
+                        // one neighbour species in the group: every pair feeds every channel (no species lookup)
+                        const bool on = (j >= s0) && (j < s1) && (one_species ? s_nu == 0 : sjs[j] == s_nu);
                         const double av = on ? grow[j] : 0.0;
 #pragma unroll
                         for (int nb = 0; nb < NBY; nb++)
@@ -235,7 +241,7 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
             }
             n2 = warp_sum(n2);
             for (int p = gr.P + lane; p < gr.K; p += 32) brow[p] = 0.0;  // zero padding up to K
-            if (lane == 0) nrm_out[lrow] = sqrt(n2);                     // no neighbours: B = 0, ||B|| = 0 (R8)
+            if (lane == 0) nrm_out[lrow] = n2;  // ||B||^2 (the consumers need 1/||B||^2); no neighbours: 0 (R8)
             __syncwarp();
             for (int c = lane; c < Nc8 * AS; c += 32) As[c] = 0.0;
             __syncwarp();

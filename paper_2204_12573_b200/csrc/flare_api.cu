@@ -1239,9 +1239,10 @@ int flare_get_descriptors(flare_ctx* c, double* bhat, double* nrm) {
             double* dst = bhat + (size_t)i * P;
             for (int p = 0; p < P; p++) dst[p] = 0.0;
             // rows hold the unnormalised B; atoms without neighbours (empty group) have no row content at all (R8)
-            const double inv = (!comp.empty() && hn[r] > 0.0) ? 1.0 / hn[r] : 0.0;
+            const double nr = comp.empty() ? 0.0 : std::sqrt(hn[r]);  // the workspace holds ||B||^2
+            const double inv = nr > 0.0 ? 1.0 / nr : 0.0;
             for (size_t q = 0; q < comp.size(); q++) dst[comp[q]] = hb[(size_t)r * c->ld + q] * inv;
-            nrm[i] = comp.empty() ? 0.0 : hn[r];
+            nrm[i] = nr;
         }
     }
     return FLARE_OK;

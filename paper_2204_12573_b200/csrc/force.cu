@@ -167,8 +167,7 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
         for (int t = 1; t < gr.ntn; t++) E += part[(size_t)t * chunk_cap + lrow];
         if (want_variance)
             for (int t = 1; t < gr.ntn; t++) V += part[((size_t)max_ntn + t) * chunk_cap + lrow];
-        const double nrm = pnrm;
-        my_inv2 = (nrm > 0.0) ? 1.0 / (nrm * nrm) : 0.0;  // no neighbours: E = V = 0 (R8)
+        my_inv2 = (pnrm > 0.0) ? 1.0 / pnrm : 0.0;  // pnrm = ||B||^2; no neighbours: E = V = 0 (R8)
         my_E = E * my_inv2;
         e_s[my_k] = my_E;
         v_s[my_k] = V * my_inv2;
