@@ -190,7 +190,7 @@ struct Workspace {
     double* A = nullptr;     // [chunk][NvL2]
     double* Bh = nullptr;    // [chunk][Pld]
     double* W = nullptr;     // [chunk][Pld]
-    double* nrm = nullptr;   // [chunk]
+    double* nrm = nullptr;   // [chunk] ||B||^2 of the unnormalised rows
     double* part = nullptr;  // [2][max_ntn][chunk]  partial row-dots of the energy / variance tiles
     // ---- reductions and scalars of the analysis / thermostat kernels
     double* red = nullptr;                 // [kRedBlocksMax][9] per-block partial sums
@@ -254,7 +254,7 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
                      double dom_trigger = 0.0);  // > 0: raise Workspace::dom[kDomNeed] once an atom has moved that far
 
 // Descriptor rows [row0,row0+nrows): compact A -> ws.A, UNNORMALISED B -> bh_out (row r at (r - row0)*ld),
-// ||B|| -> nrm_out.  One launch per group.
+// ||B||^2 -> nrm_out.  One launch per group.
 void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
                      const GroupDesc* groups, int n_groups, int row0, int nrows, double* bh_out, int ld,
                      double* nrm_out, bool write_A);
