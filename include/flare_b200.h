@@ -22,7 +22,8 @@
  *   - All arrays are dense, C-contiguous: positions/forces/velocities [N][3], matrices row-major.
  *   - The caller owns every array and the workspace; the library allocates device memory only
  *     in flare_create (model matrices and tables) and frees it in flare_destroy.
- *   - All device work is enqueued on the stream given to flare_bind; device-pointer entry
+ *   - All device work is ordered on the stream given to flare_bind (inside an evaluation the launches of the small
+ *     quadratic-form groups run on a library-owned side stream that forks from and joins back into it); device-pointer entry
  *     points are asynchronous (results valid after the caller synchronises that stream) unless
  *     stated otherwise.  *_host entry points and the flare_get_* hooks synchronise.
  *   - Results are in the CALLER's atom order although atoms are cell-sorted internally.

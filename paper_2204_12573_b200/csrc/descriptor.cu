@@ -273,9 +273,11 @@ void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& y
                      const GroupDesc* groups, int n_groups, int row0, int nrows, double* bh_out, int ld,
                      double* nrm_out, bool write_A) {
     if (nrows <= 0) return;
+    L.fork();
     for (int gi = 0; gi < n_groups; gi++) {
         if (groups[gi].P == 0) continue;  // no neighbours: no descriptor (R8); nothing downstream reads these rows
         const GroupRun gr = make_group_run(groups[gi], gi, row0, nrows);
+        L.select(gi);
 #define FLARE_CASE(LM)                                                                                   \
     case LM:                                                                                             \
         if (bs.n_max <= 8) launch_descriptor<LM, 8>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A);       \
@@ -288,6 +290,7 @@ void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& y
         }
 #undef FLARE_CASE
     }
+    L.join();
 }
 
 }  // namespace flare

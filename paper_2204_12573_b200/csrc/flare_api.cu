@@ -101,6 +101,10 @@ struct flare_ctx {
     bool capturing = false;
     int64_t graph_launches = 0;         // kernels per replay
     int64_t graph_replays = 0;
+    // side stream on which the per-group launches of the small groups run beside the large one (kernels.cuh)
+    cudaStream_t side_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int* h_group_start = nullptr;  // pinned [kMaxGroups + 1]: group offsets of the previous evaluation (scheduling hint)
     PhaseEvents phases[FLARE_N_PHASES];
     std::string err;
 };
@@ -112,6 +116,16 @@ Launcher make_launcher(flare_ctx* c) {
     L.stream = c->stream;
     L.launch_count = &c->launches;
     L.cache = &c->launch_cache;
+    if (c->side_stream && c->h_group_start && c->n_groups > 1) {
+        L.side = c->side_stream;
+        L.ev_fork = c->ev_fork;
+        L.ev_join = c->ev_join;
+        int best = 0;
+        for (int g = 0; g < c->n_groups; g++) {
+            const int rows = c->h_group_start[g + 1] - c->h_group_start[g];
+            if (rows > best) { best = rows; L.big_group = g; }
+        }
+    }
     return L;
 }
 
@@ -417,6 +431,9 @@ int evaluate(flare_ctx* c, Launcher& L, const double* pos, const int* types, dou
         build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups, eff_skin(c),
                         c->list_valid, c->dom_active ? c->dom_trigger : 0.0);
         if (eff_skin(c) > 0.0) c->list_valid = true;
+        // group sizes of this evaluation -> pinned host memory, read (without waiting) when the NEXT evaluation is enqueued
+        if (c->h_group_start && !c->capturing && L.err == cudaSuccess)
+            cudaMemcpyAsync(c->h_group_start, c->ws.group_start, sizeof(int) * (c->n_groups + 1), cudaMemcpyDeviceToHost, L.stream);
     }
     for (int row0 = 0; row0 < n; row0 += c->chunk_cap) {
         const int nrows = std::min(c->chunk_cap, n - row0);
@@ -513,6 +530,15 @@ int flare_create(flare_ctx** out, int n_species, const double* mass_amu, int n_m
         for (int s = 0; s < n_species; s++) hm[s] = mass_amu[s];
         rc = upload(c, hm, &c->d_mass);
     }
+    if (rc == FLARE_OK) {
+        if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+            cudaMallocHost(&c->h_group_start, sizeof(int) * (kMaxGroups + 1)) != cudaSuccess)
+            rc = FLARE_ERR_CUDA;
+        else
+            memset(c->h_group_start, 0, sizeof(int) * (kMaxGroups + 1));
+    }
     if (rc != FLARE_OK) { flare_destroy(c); return rc; }
     c->h_accel.assign(kMaxSpecies, 0.0);
     *out = c;
@@ -523,6 +549,10 @@ void flare_destroy(flare_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     drop_step_graph(c);
+    if (c->side_stream) cudaStreamDestroy(c->side_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->h_group_start) cudaFreeHost(c->h_group_start);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->body_stream) cudaStreamDestroy(c->body_stream);
     for (void* p : c->dev_allocs) cudaFree(p);

@@ -367,8 +367,10 @@ void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, 
                   const GroupDesc* groups, int n_groups, int row0, int nrows, int ld, int chunk_cap, int max_ntn,
                   bool want_variance) {
     if (nrows <= 0) return;
+    L.fork();
     for (int gi = 0; gi < n_groups; gi++) {
         const GroupRun gr = make_group_run(groups[gi], gi, row0, nrows);
+        L.select(gi);
 #define FLARE_CASE(LM)                                                                                        \
     case LM:                                                                                                  \
         if (bs.n_max <= 8) launch_backprop<LM, 8>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);       \
@@ -381,6 +383,7 @@ void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, 
         }
 #undef FLARE_CASE
     }
+    L.join();
 }
 
 // ------------------------------------------------------------------ a7: atomics-free gather

@@ -54,6 +54,10 @@ struct Launcher {
     cudaError_t err = cudaSuccess;
     const char* err_where = nullptr;
 
+    void fail_here(cudaError_t e, const char* where) {
+        if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = where; }
+    }
+
     // raise the kernel's dynamic shared-memory limit (needed above 48 KB) once per context and size
     template <class... KArgs>
     void ensure_smem(void (*kernel)(KArgs...), size_t bytes) {
@@ -88,6 +92,30 @@ struct Launcher {
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = "kernel launch"; }
     }
+    // ---- side stream: the per-group launches of a phase are independent (disjoint rows), so the groups with few rows
+    // run beside the large one instead of after it (their kernels cannot fill the GPU by themselves)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int big_group = -1;  // group expected to hold most rows (a scheduling hint only); -1: no overlap
+    cudaStream_t main_stream = nullptr;
+    bool forked = false;
+    void fork() {
+        if (!side || big_group < 0 || err != cudaSuccess) return;
+        fail_here(cudaEventRecord(ev_fork, stream), "cudaEventRecord(fork)");
+        fail_here(cudaStreamWaitEvent(side, ev_fork, 0), "cudaStreamWaitEvent(fork)");
+        main_stream = stream;
+        forked = err == cudaSuccess;
+    }
+    void select(int group) {  // the stream the launches of this group go to
+        if (forked) stream = (group == big_group) ? main_stream : side;
+    }
+    void join() {
+        if (!forked) return;
+        stream = main_stream;
+        forked = false;
+        fail_here(cudaEventRecord(ev_join, side), "cudaEventRecord(join)");
+        fail_here(cudaStreamWaitEvent(stream, ev_join, 0), "cudaStreamWaitEvent(join)");
+    }
     void memset(void* p, int v, size_t bytes) {
         if (bytes == 0 || err != cudaSuccess) return;
         cudaError_t e = cudaMemsetAsync(p, v, bytes, stream);
@@ -102,9 +130,6 @@ struct Launcher {
     cudaStream_t body_stream = nullptr;  // side stream the IF body is captured on
     cudaStream_t outer_stream = nullptr;
     cudaGraphNode_t cond_node = nullptr;
-    void fail_here(cudaError_t e, const char* where) {
-        if (e != cudaSuccess && err == cudaSuccess) { err = e; err_where = where; }
-    }
     cudaGraphConditionalHandle cond_handle() {
         cudaGraphConditionalHandle h = 0;
         if (err != cudaSuccess) return h;
