@@ -69,7 +69,7 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     int* sjs = reinterpret_cast<int*>(As + Nc8 * AS);            // [32] compact species of the staged pairs
     const bool one_species = gr.nsp == 1;
     // zeroed once per warp: the staged rows keep finite values from then on (idle lanes' columns are masked by a zero
-    // operand, which needs a finite partner), the Y padding rows stay zero, and A is re-zeroed after every atom
+    // operand, which needs a finite partner), the Y padding rows stay zero, and the first segment of an atom overwrites A
     if ((blockIdx.x * kDescWarps + warp) * kDescTA < ge_ - gs_)
         for (int c = lane; c < (NMAXP + SM::YR) * kPS + Nc8 * AS; c += 32) gsm[c] = 0.0;
     // the grid is capped (a launch for a group with few or no rows costs next to nothing): a warp strides over its blocks
@@ -178,15 +178,21 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
                         for (int nb = 0; nb < NBY; nb++)
                             dmma884_d(acc[nb][0], acc[nb][1], av, ysm[(nb * 8 + g8) * kPS + j]);
                     }
+                    // the first segment of an atom overwrites A (nothing to re-zero between atoms); only an atom that
+                    // continues from the previous pass accumulates
                     double* arow = As + cnu * AS + 2 * t4;
+                    const bool first_seg = a_start >= p0;
 #pragma unroll
                     for (int nb = 0; nb < NBY; nb++) {
                         double2* dst = reinterpret_cast<double2*>(arow + nb * 8);
-                        double2 v = *dst;
-                        v.x += acc[nb][0]; v.y += acc[nb][1];
+                        double2 v = make_double2(acc[nb][0], acc[nb][1]);
+                        if (!first_seg) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
                         *dst = v;
                     }
                 }
+                __syncwarp();
+            } else if (a_end == a_start) {  // an atom without neighbours (cannot be in a group with P > 0; kept for safety)
+                for (int c = lane; c < Nc8 * AS; c += 32) As[c] = 0.0;
                 __syncwarp();
             }
             if (a_end > p0 + 32) break;  // the atom continues in the next pass
@@ -194,9 +200,16 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
             const int lrow = lrow0 + a;
             if (A_out) {
                 double* arow = A_out + (size_t)lrow * bs.NvL2;
-                for (int c = lane; c < Nc * L2; c += 32) {
-                    const int nu = c / L2;
-                    arow[c] = As[nu * AS + (c - nu * L2)];
+                if constexpr (L2 % 2 == 0) {
+                    for (int c = 2 * lane; c < Nc * L2; c += 64) {
+                        const int nu = c / L2;
+                        *reinterpret_cast<double2*>(arow + c) = *reinterpret_cast<const double2*>(As + nu * AS + (c - nu * L2));
+                    }
+                } else {
+                    for (int c = lane; c < Nc * L2; c += 32) {
+                        const int nu = c / L2;
+                        arow[c] = As[nu * AS + (c - nu * L2)];
+                    }
                 }
             }
             double* brow = b_out + (size_t)lrow * ld;
@@ -242,8 +255,6 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
             n2 = warp_sum(n2);
             for (int p = gr.P + lane; p < gr.K; p += 32) brow[p] = 0.0;  // zero padding up to K
             if (lane == 0) nrm_out[lrow] = n2;  // ||B||^2 (the consumers need 1/||B||^2); no neighbours: 0 (R8)
-            __syncwarp();
-            for (int c = lane; c < Nc8 * AS; c += 32) As[c] = 0.0;
             __syncwarp();
             a++;
         }
