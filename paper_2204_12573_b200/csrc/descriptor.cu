@@ -23,7 +23,7 @@
 namespace flare {
 
 constexpr int kDescWarps = 4;
-constexpr int kDescTA = 8;  // atoms per warp
+constexpr int kDescTA = 8;  // atoms per warp (upper bound; small systems take fewer, see launch_descriptor)
 constexpr int kPS = 36;     // pair stride of the staged rows (= 4 mod 16)
 
 __host__ __device__ constexpr int pad4mod16(int n) {  // smallest m >= n with m % 16 == 4
@@ -46,7 +46,7 @@ __device__ __forceinline__ void dmma884_d(double& c0, double& c1, double a, doub
 
 template <int LMAX, int NMAXP>
 __global__ void __launch_bounds__(kDescWarps * 32)
-k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
+k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restrict__ atoms, const int* __restrict__ nbr_cnt,
              const int* __restrict__ nbr_idx, int mmax, const int* __restrict__ atom_of_row,
              const int* __restrict__ group_start, double* __restrict__ A_out, double* __restrict__ b_out, int ld,
              double* __restrict__ nrm_out) {
@@ -70,12 +70,12 @@ k_descriptor(Grid g, Basis bs, YNorm yn, GroupRun gr, const AtomS* __restrict__ 
     const bool one_species = gr.nsp == 1;
     // zeroed once per warp: the staged rows keep finite values from then on (idle lanes' columns are masked by a zero
     // operand, which needs a finite partner), the Y padding rows stay zero, and the first segment of an atom overwrites A
-    if ((blockIdx.x * kDescWarps + warp) * kDescTA < ge_ - gs_)
+    if ((blockIdx.x * kDescWarps + warp) * ta < ge_ - gs_)
         for (int c = lane; c < (NMAXP + SM::YR) * kPS + Nc8 * AS; c += 32) gsm[c] = 0.0;
     // the grid is capped (a launch for a group with few or no rows costs next to nothing): a warp strides over its blocks
-    for (int r0 = (blockIdx.x * kDescWarps + warp) * kDescTA; r0 < ge_ - gs_; r0 += gridDim.x * kDescWarps * kDescTA) {
+    for (int r0 = (blockIdx.x * kDescWarps + warp) * ta; r0 < ge_ - gs_; r0 += gridDim.x * kDescWarps * ta) {
     // warps are independent: only __syncwarp below
-    const int na = min(kDescTA, ge_ - gs_ - r0);
+    const int na = min(ta, ge_ - gs_ - r0);
     const int lrow0 = gs_ - gr.row0 + r0;  // chunk-local row of the warp's first atom
 
     // per-lane atom bookkeeping (lanes 0..na-1), inclusive scan of the neighbour counts
@@ -272,10 +272,11 @@ static void launch_descriptor(Launcher& L, const Grid& g, const Basis& bs, const
     const int Nc8 = (gr.Nc + 7) & ~7;
     const size_t smem = sizeof(double) * kDescWarps * (size_t)SM::warp_doubles(Nc8);
     L.ensure_smem(k_descriptor<LMAX, NMAXP>, smem);
-    const int per_cta = kDescWarps * kDescTA;
+    const int ta = small_system_ta(gr.nrows, kDescWarps, kDescTA);
+    const int per_cta = kDescWarps * ta;
     const int grid = std::min((gr.nrows + per_cta - 1) / per_cta, 148 * 32);
     L.launch(k_descriptor<LMAX, NMAXP>, dim3(grid), dim3(kDescWarps * 32), smem, g, bs, yn,
-             gr, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
+             gr, ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const int*)ws.group_start, write_A ? ws.A : (double*)nullptr, bh_out, ld,
              nrm_out);
 }

@@ -344,6 +344,7 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
         target = target > 4 ? 4 : (target < 1 ? 1 : target);
         while (ta > 1 && cta_bytes(ta) * target > sm_bytes) ta--;
     }
+    ta = std::min(ta, small_system_ta(gr.nrows, kBpWarps, kBpMaxTA));
     // warps per CTA: as many of kBpWarps as fit the 227 KB of shared memory a CTA can have (large (n_max, l_max))
     const size_t per_warp = sizeof(double) * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
     int warps = kBpWarps;

@@ -247,6 +247,17 @@ struct GroupDesc {
     unsigned sidx = 0;              // 4 bits per species: its rank within mask (15 = absent)
 };
 
+// Atoms per warp of the per-atom kernels: packing the neighbour lists of several atoms into 32-pair passes fills the
+// lanes, but a small system is bound by the latency of one warp's chain, not by throughput: with fewer than ~2 warps
+// per SM sub-partition at the full count, take fewer atoms per warp so that more warps (and SMs) share the rows.
+inline int small_system_ta(int nrows, int warps_per_cta, int ta_max) {
+    const int warps_wanted = 148 * 4 * 2;
+    int ta = ta_max;
+    while (ta > 1 && (nrows + ta - 1) / ta < warps_wanted) ta--;
+    (void)warps_per_cta;
+    return ta;
+}
+
 // What a per-(chunk, group) launch of the per-atom kernels needs (passed by value).
 struct GroupRun {
     int g;          // group id: rows group_start[g] .. group_start[g+1], intersected with the chunk

@@ -516,8 +516,11 @@ static void launch_qform_res(Launcher& L, const QrArgs& a, int sm_count) {
     constexpr int warps = kQrWarps * (3 - kQrH);
     const size_t smem = sizeof(double) * (size_t)K * (K + 4);
     L.ensure_smem(k_qform_res<K16, kQrH>, smem);
+    // one CTA per SM; for small systems one CTA per block and matrix rather than 16 blocks per CTA: a block is ~5 us of
+    // DMMA pipe time on one SM sub-partition, and a small step is bound by exactly such latencies
     const long long items = ((long long)a.nrows + 8 * kQrH - 1) / (8 * kQrH);
-    const int grid = (int)std::max<long long>(1, std::min<long long>(sm_count, (items + warps - 1) / warps));
+    (void)warps;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(sm_count, items * a.n_mat));
     L.launch(k_qform_res<K16, kQrH>, dim3(grid), dim3(warps * 32), smem, a);
 }
 
