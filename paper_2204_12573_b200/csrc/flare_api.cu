@@ -306,6 +306,29 @@ struct Carver {
     }
 };
 
+// Small systems: the tile kernel of the large matrices (K > 144) is latency-bound there -- a 64 x 112 tile is
+// 34 slabs of K = 544 run back to back on one SM -- so below kNarrowAtoms atoms the tiles are 16 columns wide (nb = 2,
+// K / 16 tiles per matrix): many short tiles on many SMs.  The matrices keep their layout (rows = columns of the symmetric
+// matrix, K of them are always there); only the number of partial row-dots per row grows, which small systems can afford.
+constexpr int64_t kNarrowAtoms = 8192;
+constexpr int kResidentK = 144;  // largest K of the resident-matrix kernel (qform.cu)
+
+int eff_max_ntn(const flare_ctx* c, bool narrow) {
+    int m = 0;
+    for (const GroupDesc& g : c->sets[c->sparse].groups) m = std::max(m, (narrow && g.K > kResidentK) ? g.K / 16 : g.ntn);
+    return m;
+}
+
+void apply_tiling(flare_ctx* c, bool narrow) {
+    const flare_ctx::GroupSet& gs = c->sets[c->sparse];
+    for (int g = 0; g < gs.n_groups; g++) {
+        c->groups[g].nb = gs.groups[g].nb;
+        c->groups[g].ntn = gs.groups[g].ntn;
+        if (narrow && gs.groups[g].K > kResidentK) { c->groups[g].nb = 2; c->groups[g].ntn = gs.groups[g].K / 16; }
+    }
+    c->max_ntn = eff_max_ntn(c, narrow);
+}
+
 int auto_chunk(const flare_ctx* c, int64_t n) {
     if (c->chunk_opt > 0) return (int)std::min<int64_t>(std::max<int64_t>(c->chunk_opt, 1), std::max<int64_t>(n, 1));
     const double per_row = 8.0 * (c->bs.NvL2 + 2.0 * c->ld + 1 + 2.0 * c->max_ntn);
@@ -358,7 +381,7 @@ size_t carve(const flare_ctx* c, int64_t n, char* base, Workspace* ws, int* chun
     w.Bh = cv.take<double>((size_t)chunk * c->ld);
     w.W = cv.take<double>((size_t)chunk * c->ld);
     w.nrm = cv.take<double>(chunk);
-    w.part = cv.take<double>((size_t)2 * std::max(c->max_ntn, 1) * chunk);
+    w.part = cv.take<double>((size_t)2 * std::max(eff_max_ntn(c, n <= kNarrowAtoms), 1) * chunk);
     w.red = cv.take<double>((size_t)kRedBlocksMax * 9);
     w.scal = cv.take<double>(16);
     w.ascal = cv.take<unsigned long long>(18);
@@ -640,6 +663,7 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     if (bytes < need) return fail(c, FLARE_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than flare_workspace_bytes");
     FLARE_CUDA(c, cudaSetDevice(c->device));
     carve(c, n_atoms, static_cast<char*>(workspace), &c->ws, &c->chunk_cap, &c->n_cells_cap);
+    apply_tiling(c, n_atoms <= kNarrowAtoms);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->n = c->n_cap = n_atoms;
     c->dom_active = false;
