@@ -290,12 +290,12 @@ static void launch_qform(Launcher& L, const QfArgs& a, int sm_count, long long m
 // For the small matrices (P = 144 after the species-sparse compaction: 98 % of the rows of the H2/Pt(111)
 // workloads) the whole symmetric matrix fits in one SM's shared memory (144 x 148 doubles = 170 KB).  One persistent
 // CTA per SM keeps ONE matrix (beta or Sigma) resident -- fetched once by per-row bulk copies (TMA, completion on an
-// mbarrier) -- and its 8 warps work independently: a warp takes a block of 16 rows from a device queue, loads those
-// rows of B straight into registers in A-fragment layout (16 x K doubles = 72 per lane at K = 144), and runs the
-// whole K loop out of registers and the resident matrix, 48 output columns at a time.  No operand ever waits on
+// mbarrier) -- and its 16 warps work independently: a warp takes a block of 8 rows from a device queue, loads those
+// rows of B straight into registers in A-fragment layout (8 x K doubles = 36 per lane at K = 144), and runs the
+// whole K loop out of registers and the resident matrix, 48 output columns at a time (H = 2: 16-row blocks, 8 warps).  No operand ever waits on
 // another warp: there is no barrier in the steady state, and a row's E (or V) is complete inside one warp, so no
 // partial row-dots are left for later.  CTAs that run out of blocks of their matrix switch to the other one.
-constexpr int kQrWarps = 8;
+constexpr int kQrWarps = 8;  // warps per CTA at H = 2; 16 at H = 1
 constexpr int kQrNB = 6;  // n8 blocks (48 columns) per pass: 24 accumulator doubles per lane
 
 struct QrArgs {
