@@ -663,6 +663,45 @@ k_group_assign(int n, int S, int sparse, int n_groups, const AtomS* __restrict__
     }
 }
 
+// n <= kGroupBlock: histogram, scan and assignment in one block and one launch (a small step is bound by the latency of
+// its chain of tiny kernels); same row order as the three-kernel version
+__global__ void __launch_bounds__(kGroupBlock)
+k_group_small(int n, int S, int sparse, int n_groups, const AtomS* __restrict__ atoms,
+              const unsigned char* __restrict__ nmask, int* __restrict__ group_start, int* __restrict__ row_of,
+              int* __restrict__ atom_of_row, unsigned char* __restrict__ gid_out) {
+    __shared__ int wcnt[32][kMaxGroups];
+    __shared__ int start[kMaxGroups + 1];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int t = threadIdx.x; t < 32 * kMaxGroups; t += blockDim.x) (&wcnt[0][0])[t] = 0;
+    __syncthreads();
+    const int k = threadIdx.x;
+    const int gid = (k < n) ? group_of(atoms[k].type, nmask[k], S, sparse) : -1;
+    const unsigned peers = __match_any_sync(kFull, gid);
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    if (gid >= 0 && rank == 0) wcnt[w][gid] = __popc(peers);
+    __syncthreads();
+    if (threadIdx.x < n_groups) {  // total of each group ...
+        int tot = 0;
+        for (int ww = 0; ww < 32; ww++) tot += wcnt[ww][threadIdx.x];
+        start[threadIdx.x + 1] = tot;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {  // ... laid out one after another
+        start[0] = 0;
+        for (int gq = 0; gq < n_groups; gq++) start[gq + 1] += start[gq];
+        for (int gq = 0; gq <= n_groups; gq++) group_start[gq] = start[gq];
+    }
+    __syncthreads();
+    if (gid >= 0) {
+        int before = 0;
+        for (int ww = 0; ww < w; ww++) before += wcnt[ww][gid];
+        const int row = start[gid] + before + rank;
+        row_of[k] = row;
+        atom_of_row[row] = k;
+        gid_out[k] = (unsigned char)gid;
+    }
+}
+
 // ------------------------------------------------------------------ host-side driver of a1
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
                      const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid,
@@ -732,6 +771,11 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
                  (const int*)ws.skin_idx, (const unsigned char*)ws.skin_rev, (const unsigned long long*)ws.hitmask, ws.rev);
     }
     const int ngb = (n + kGroupBlock - 1) / kGroupBlock;
+    if (ngb == 1) {
+        L.launch(k_group_small, dim3(1), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
+                 (const unsigned char*)ws.nmask, ws.group_start, ws.row_of, ws.atom_of_row, ws.gid);
+        return;
+    }
     L.launch(k_group_hist, dim3(ngb), dim3(kGroupBlock), 0, n, bs.S, sparse, n_groups, (const AtomS*)ws.atoms,
              (const unsigned char*)ws.nmask, ws.group_hist);
     L.launch(k_group_scan, dim3(1), dim3(32 * 32), 0, ngb, n_groups, ws.group_hist, ws.group_start);

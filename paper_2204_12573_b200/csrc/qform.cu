@@ -367,11 +367,12 @@ __global__ void __launch_bounds__(kQrWarps * 32 * (3 - H), 1) k_qform_res(QrArgs
     __syncthreads();
     for (int round = 0; round < 2; round++) {
         // ---- fetch the matrix: K bulk copies of one row each into the padded rows
-        if (tid == 0) {
+        // (one row per thread: issued by one thread alone the K copies take longer than a small system's whole K loop)
+        if (tid < K) {
             asm volatile("fence.proxy.async.shared::cta;\n" ::);  // earlier generic-proxy reads of Ms are done (syncthreads)
             const double* M = mat == 0 ? a.beta : a.sigma;
-            qr_mbar_expect(&bar, (unsigned)(K * K * sizeof(double)));
-            for (int n = 0; n < K; n++) qr_bulk_row(Ms + n * MS, M + (size_t)n * K, (unsigned)(K * sizeof(double)), &bar);
+            if (tid == 0) qr_mbar_expect(&bar, (unsigned)(K * K * sizeof(double)));
+            qr_bulk_row(Ms + tid * MS, M + (size_t)tid * K, (unsigned)(K * sizeof(double)), &bar);
         }
         qr_mbar_wait(&bar, phase);
         phase ^= 1u;
