@@ -28,8 +28,10 @@ struct BpSmem {
     static constexpr int AS = bp_pad4mod16(L2);    // row stride of the staged A (conflict-free operand loads)
     static constexpr int GB = L2 * NMAXP + 2;      // G^T block of one (atom, species): [L2][NMAXP] + bank shift
     // G^T of ta atoms + double-buffered [A | W | B] rows of one atom (filled by cp.async one atom ahead)
-    __host__ __device__ static int warp_doubles(int ta, int nsp, int Nc8, int K) {
-        return (ta * nsp * GB + 2 * (Nc8 * AS + 2 * K) + 1) & ~1;  // even: every warp's region stays 16-byte aligned
+    // staged: W and B rows go through shared memory too (small K); otherwise only A does and dE/dB is formed from global
+    // memory (large K: the rows would cost resident warps)
+    __host__ __device__ static int warp_doubles(int ta, int nsp, int Nc8, int K, bool staged) {
+        return (ta * nsp * GB + 2 * (Nc8 * AS + (staged ? 2 * K : 0)) + 1) & ~1;  // even: 16-byte aligned regions
     }
 };
 
@@ -75,7 +77,7 @@ __device__ __forceinline__ void radial_fixed(int n_max, double r, double inv_rc,
 // One launch per (chunk, group).  A warp owns `ta` consecutive rows: phase 1 forms E, V, c = dE/dB and
 // G = dE/dA of each of its atoms (G on the tensor pipe), phase 2 walks over the concatenated neighbour
 // lists of those atoms, one pair per lane, so that the basis gradients run with nearly full lanes.
-template <int LMAX, int NMAXP>
+template <int LMAX, int NMAXP, bool STAGED>
 __global__ void __launch_bounds__(kBpWarps * 32, 4)
 k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restrict__ atoms,
            const int* __restrict__ nbr_cnt, const int* __restrict__ nbr_idx, int mmax,
@@ -102,9 +104,9 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     const int g8 = lane >> 2, t4 = lane & 3;
     const int n_max = bs.n_max;
     const int Nc = gr.Nc, Nc8 = (Nc + 7) & ~7, nmb = Nc8 >> 3;
-    double* Gt = smem + (size_t)warp * SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);  // [ta][nsp][GB]
+    double* Gt = smem + (size_t)warp * SM::warp_doubles(ta, gr.nsp, Nc8, gr.K, STAGED);  // [ta][nsp][GB]
     double* rows = Gt + ta * gr.nsp * GB;  // [2][ A [Nc8][AS] | W [K] | B [K] ]
-    const int row_doubles = Nc8 * AS + 2 * gr.K;
+    const int row_doubles = Nc8 * AS + (STAGED ? 2 * gr.K : 0);
     // the first loads of the block are issued before anything else: the atom of each row, and (lane a for atom a) the
     // first tile partials and ||B|| that phase 1 starts from
     int my_k = 0, my_cnt = 0;
@@ -188,12 +190,14 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
                 bp_cp_async8(As + nu * AS + (c - nu * L2), arow + c);
             }
         }
-        double* Ws = As + Nc8 * AS;
-        const double* wrow = W + (size_t)lrow * ld;
-        const double* brow = Braw + (size_t)lrow * ld;
-        for (int c = 2 * lane; c < gr.K; c += 64) {
-            bp_cp_async16(Ws + c, wrow + c);
-            bp_cp_async16(Ws + gr.K + c, brow + c);
+        if constexpr (STAGED) {
+            double* Ws = As + Nc8 * AS;
+            const double* wrow = W + (size_t)lrow * ld;
+            const double* brow = Braw + (size_t)lrow * ld;
+            for (int c = 2 * lane; c < gr.K; c += 64) {
+                bp_cp_async16(Ws + c, wrow + c);
+                bp_cp_async16(Ws + gr.K + c, brow + c);
+            }
         }
     };
     if (gr.P > 0) issue_rows(0, 0);
@@ -206,8 +210,9 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
         const double E = __shfl_sync(kFull, my_E, a);
         const double two_inv2 = 2.0 * __shfl_sync(kFull, my_inv2, a);
         const double* As = rows + (a & 1) * row_doubles;
-        const double* Ws = As + Nc8 * AS;
-        const double* Bs = Ws + gr.K;
+        // W and B of this atom: staged in shared memory, or (large K) read where they are, in global memory
+        const double* Ws = STAGED ? As + Nc8 * AS : W + (size_t)(lrow0 + a) * ld;
+        const double* Bs = STAGED ? Ws + gr.K : Braw + (size_t)(lrow0 + a) * ld;
 
         // G[cnu1, (l,m)] = sum_cnu2 C_l[cnu1,cnu2] A[cnu2,(l,m)], C_l[cnu1,cnu2] = c[q(cnu1,cnu2) L + l]: per l a small
         // symmetric-matrix product on the tensor pipe.  A-operand (row cnu1 = 8mb+g8, col cnu2 = k0+t4),
@@ -327,26 +332,32 @@ k_backprop(Grid g, Basis bs, YNorm yn, GroupRun gr, int ta, const AtomS* __restr
     }  // blocks of this warp
 }
 
-template <int LMAX, int NMAXP>
-static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
+template <int LMAX, int NMAXP, bool STAGED>
+static void launch_backprop_(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
                             int mmax, const GroupRun& gr, int ld, int chunk_cap, int max_ntn, bool want_variance) {
     using SM = BpSmem<LMAX, NMAXP>;
     const int Nc8 = (gr.Nc + 7) & ~7;
-    // atoms per warp (1..8): the most that do not cost resident CTAs.  With one atom per warp ctas1 CTAs of kBpWarps warps
-    // fit in an SM's shared memory (at most 4 matter: 128 registers per thread); more atoms per warp pack more pairs
-    // into each 32-lane pass, so take the largest count that still lets min(ctas1, 4) CTAs fit.
+    // atoms per warp (1..8) against resident CTAs per SM (1..4: 128 registers per thread): more atoms per warp pack more
+    // pairs into each 32-lane pass, but their G^T blocks cost shared memory.  Take the most CTAs that still leave at
+    // least two atoms per warp, and then as many atoms as fit (measured: (8,3) 4 CTAs x 6 atoms, (10,4) 4 x 2 beats
+    // 2 x 7, (12,6) 2 x 3 beats 3 x 1).
     int ta = kBpMaxTA;
     if (gr.nsp > 0) {
         const size_t sm_bytes = 228 * 1024;  // per SM
         // + 1 KB: the shared memory the system reserves per resident CTA
-        auto cta_bytes = [&](int t) { return sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(t, gr.nsp, Nc8, gr.K) + 1024; };
-        int target = (int)(sm_bytes / cta_bytes(1));
-        target = target > 4 ? 4 : (target < 1 ? 1 : target);
-        while (ta > 1 && cta_bytes(ta) * target > sm_bytes) ta--;
+        auto cta_bytes = [&](int t) { return sizeof(double) * kBpWarps * (size_t)SM::warp_doubles(t, gr.nsp, Nc8, gr.K, STAGED) + 1024; };
+        auto fit = [&](int target) {
+            int t = kBpMaxTA;
+            while (t > 1 && cta_bytes(t) * target > sm_bytes) t--;
+            return t;
+        };
+        int target = 4;
+        while (target > 1 && (cta_bytes(1) * target > sm_bytes || fit(target) < 2)) target--;
+        ta = fit(target);
     }
     ta = std::min(ta, small_system_ta(gr.nrows, kBpWarps, kBpMaxTA));
     // warps per CTA: as many of kBpWarps as fit the 227 KB of shared memory a CTA can have (large (n_max, l_max))
-    const size_t per_warp = sizeof(double) * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K);
+    const size_t per_warp = sizeof(double) * (size_t)SM::warp_doubles(ta, gr.nsp, Nc8, gr.K, STAGED);
     int warps = kBpWarps;
     while (warps > 1 && per_warp * warps > 220 * 1024) warps--;
     const size_t smem = per_warp * warps;
@@ -354,14 +365,23 @@ static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const Y
         if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.err_where = "back-propagation: descriptor too large for shared memory"; }
         return;
     }
-    L.ensure_smem(k_backprop<LMAX, NMAXP>, smem);
+    L.ensure_smem(k_backprop<LMAX, NMAXP, STAGED>, smem);
     const int per_cta = warps * ta;
     const int grid = std::min((gr.nrows + per_cta - 1) / per_cta, 148 * 32);
-    L.launch(k_backprop<LMAX, NMAXP>, dim3(grid), dim3(warps * 32), smem, g, bs, yn, gr,
+    L.launch(k_backprop<LMAX, NMAXP, STAGED>, dim3(grid), dim3(warps * 32), smem, g, bs, yn, gr,
              ta, (const AtomS*)ws.atoms, (const int*)ws.nbr_cnt, (const int*)ws.nbr_idx, mmax,
              (const int*)ws.atom_of_row, (const int*)ws.group_start, (const double*)ws.A, (const double*)ws.Bh,
              (const double*)ws.W, (const double*)ws.nrm, (const double*)ws.part, ld, chunk_cap, max_ntn,
              want_variance ? 1 : 0, ws.pairf, ws.e_s, ws.v_s);
+}
+
+// W and B rows staged through shared memory only while they are small (K <= 160: the single-species groups of (8,3));
+// for larger K the 2 x 2K doubles per warp would cost resident warps (one CTA of 4 warps per SM at (12,6))
+template <int LMAX, int NMAXP>
+static void launch_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws,
+                            int mmax, const GroupRun& gr, int ld, int chunk_cap, int max_ntn, bool want_variance) {
+    if (gr.K <= 160) launch_backprop_<LMAX, NMAXP, true>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);
+    else launch_backprop_<LMAX, NMAXP, false>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);
 }
 
 void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, const Workspace& ws, int mmax,
