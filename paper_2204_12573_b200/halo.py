@@ -109,11 +109,12 @@ class DomainDecomposition:
 
     def __init__(self, engine: Engine, box, pbc, r_cut_max: float, grid=None, axes=(0, 1), halo_skin: float = 1.2,
                  lag: int = 2, border_capacity: int | None = None, migrate_capacity: int = 8192, self_halo: bool = False,
-                 group=None):
+                 group=None, rank: int | None = None, world: int | None = None):
         self.engine = engine
         self.group = group
-        self.world = dist.get_world_size(group) if dist.is_initialized() else 1
-        self.rank = dist.get_rank(group) if dist.is_initialized() else 0
+        # rank / world default to the process group's; given explicitly they describe a rank's geometry without one (tests)
+        self.world = world if world is not None else (dist.get_world_size(group) if dist.is_initialized() else 1)
+        self.rank = rank if rank is not None else (dist.get_rank(group) if dist.is_initialized() else 0)
         if grid is None:
             grid = (self.world, 1)
         if grid[0] * grid[1] != self.world:

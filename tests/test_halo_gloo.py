@@ -110,3 +110,25 @@ def test_geometry_checks():
     assert dd.phases == [] and dd.h == pytest.approx(7.2) and dd.trigger == pytest.approx(0.42)
     with pytest.raises(ValueError):
         DomainDecomposition(Engine(), np.diag([20.0, 10.0, 10.0]).reshape(9), [1, 1, 0], 3.0, grid=(2, 1))
+
+
+def test_process_grid_geometry_4x2():
+    """Rank <-> (cx, cy) mapping, mutual neighbours along both axes (periodic wrap), local frames that tile the box."""
+    from paper_2204_12573_b200.halo import DomainDecomposition, Engine
+
+    box, pbc, rc = np.diag([120.0, 60.0, 30.0]).reshape(9), [1, 1, 0], 3.0
+    dds = [DomainDecomposition(Engine(), box, pbc, rc, grid=(4, 2), halo_skin=1.0, rank=r, world=8) for r in range(8)]
+    for r, dd in enumerate(dds):
+        cx, cy = r // 2, r % 2
+        phx, phy = dd.phases
+        assert (phx["axis"], phx["p"], phx["c"], phy["axis"], phy["p"], phy["c"]) == (0, 4, cx, 1, 2, cy)
+        assert phx["lo_rank"] == ((cx - 1) % 4) * 2 + cy and phx["hi_rank"] == ((cx + 1) % 4) * 2 + cy
+        assert phy["lo_rank"] == cx * 2 + (cy - 1) % 2 and phy["hi_rank"] == cx * 2 + (cy + 1) % 2
+        # neighbours are mutual
+        assert dds[phx["hi_rank"]].phases[0]["lo_rank"] == r and dds[phy["hi_rank"]].phases[1]["lo_rank"] == r
+        # local frame: open along x and y with the owned rectangle at [h, h + w); z untouched
+        assert dd.local_pbc.tolist() == [0, 0, 0] and dd.h == pytest.approx(7.0)
+        assert dd.local_L.tolist() == pytest.approx([30.0 + 14.0, 30.0 + 14.0, 30.0])
+        assert dd.lo.tolist() == pytest.approx([cx * 30.0 - 7.0, cy * 30.0 - 7.0, 0.0])
+    with pytest.raises(ValueError):  # a domain narrower than the halo
+        DomainDecomposition(Engine(), box, pbc, rc, grid=(4, 2), halo_skin=30.0, rank=0, world=8)
