@@ -195,6 +195,36 @@ int flare_set_thermostat(flare_ctx* ctx, double xi, double eta);
 int flare_get_virial(flare_ctx* ctx, double virial[9]);
 
 /*
+ * The same virial for hosts that cannot allocate device memory and have no workspace to spare.
+ *
+ * Who needs it: a program that embeds this library and took all its device memory at start-up through its own pool
+ * (at 10 M atoms that is nearly the whole 180 GB).  Inside such a program a cudaMalloc made on its behalf may find
+ * nothing left, stalls every stream of the GPU while the driver maps memory (cudaFree does too), and is often simply
+ * forbidden -- a pressure coupling or a monitor that runs every step has no room for either.  flare_get_virial
+ * avoids allocation by taking its partial sums from the bound workspace and hands the result to the HOST after a
+ * synchronisation; this call takes NOTHING from the caller but the result buffer, and leaves it on the device:
+ *   virial_dev  [9] DEVICE doubles (row-major 3 x 3, eV), written by work enqueued on the bound stream;
+ *               valid once the caller has synchronised that stream.  Asynchronous; no device error check
+ *               (flare_check does that).
+ * Its partial sums live in one array compiled into the library: FLARE_VIRIAL_STATIC_MAX_ATOMS / 2048 rows of 9
+ * doubles = 147 456 bytes, held on every GPU that loads the library until the process ends, used or not.
+ *   - Limit: a context bound to more than FLARE_VIRIAL_STATIC_MAX_ATOMS atoms is refused with FLARE_ERR_INVALID_ARG
+ *     (flare_last_error names the limit); use flare_get_virial there.
+ *   - The array is shared by every context and stream on a GPU.  Two calls that may run at the same time on one GPU
+ *     (different streams, or contexts driven by different threads) corrupt each other's sums: order them yourself.
+ *     Calls in sequence are safe -- each overwrites exactly the rows it then reads, so nothing left by the previous
+ *     call is seen and nothing needs clearing.
+ *   - The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that GPU current;
+ *     the runtime may load the library's kernels onto the GPU at that point).  Make that first call during set-up,
+ *     before you begin any stream capture; later calls only launch two kernels.
+ *   - It never calls cudaMalloc, cudaFree or any routine that allocates device memory, on any path.
+ * Same preconditions as flare_get_virial (an evaluation has been run).  The sums are taken tile by tile (2048 atoms)
+ * in a fixed order: repeated calls agree bit for bit; against flare_get_virial, whose order differs, to rounding.
+ */
+#define FLARE_VIRIAL_STATIC_MAX_ATOMS 4194304
+int flare_virial_static(flare_ctx* ctx, double* virial_dev);
+
+/*
  * On-the-fly analysis of the last evaluation, as in the paper's production run:
  *   max_unc     max_i sqrt(max(V_i, 0)) (the "maximum uncertainty"); n_above = #{i : sqrt(V_i) > unc_threshold}
  *               (both need an evaluation with variances, else FLARE_ERR_INVALID_ARG)

@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libflare_b200.so")
 PROBES_LIB = os.path.join(HERE, "libflare_probes.so")  # bench hooks (include/flare_probes.h), a library of their own
-SOURCES = ["flare_api.cu", "neighbor.cu", "descriptor.cu", "qform.cu", "force.cu", "integrate.cu", "analysis.cu", "domain.cu"]
+SOURCES = ["flare_api.cu", "neighbor.cu", "descriptor.cu", "qform.cu", "force.cu", "integrate.cu", "analysis.cu", "domain.cu", "virial_static.cu"]
 HEADERS = ["common.cuh", "basis.cuh", "kernels.cuh", os.path.join("..", "..", "include", "flare_b200.h"),
            os.path.join("..", "..", "include", "flare_probes.h")]
 NVCC = os.environ.get("NVCC", "nvcc")

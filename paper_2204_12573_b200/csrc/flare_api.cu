@@ -1168,6 +1168,23 @@ int flare_get_virial(flare_ctx* c, double virial[9]) {
     return flare_check(c);
 }
 
+int flare_virial_static(flare_ctx* c, double* virial_dev) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (!virial_dev) return fail(c, FLARE_ERR_INVALID_ARG, "virial_dev is null");
+    static_assert(FLARE_VIRIAL_STATIC_MAX_ATOMS == flare::kVirialStaticMaxAtoms, "header constant out of step");
+    if (c->n > (int64_t)FLARE_VIRIAL_STATIC_MAX_ATOMS)
+        return fail(c, FLARE_ERR_INVALID_ARG,
+                    "flare_virial_static: " + std::to_string(c->n) + " atoms exceed the static scratch array's limit of " +
+                        std::to_string((int64_t)FLARE_VIRIAL_STATIC_MAX_ATOMS) + " atoms; use flare_get_virial");
+    if (!c->pairf_valid) return fail(c, FLARE_ERR_NOT_BOUND, "no evaluation has been run");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    Launcher L = make_launcher(c);
+    const cudaError_t e = run_virial_static(L, c->device, c->grid, c->ws, (int)c->n, c->mmax, virial_dev);
+    if (e != cudaSuccess) return cuda_fail(c, e, L.err_where ? L.err_where : "flare_virial_static");
+    return FLARE_OK;
+}
+
 int flare_analyze(flare_ctx* c, double unc_threshold, int species_a, int species_b, double r_coord, double* max_unc,
                   int64_t* n_above, int32_t* coord, int64_t* coord_hist) {
     int rc = need_bound(c);

@@ -316,6 +316,12 @@ void run_analyze(Launcher& L, const Grid& g, const Workspace& ws, int n, int mma
 void run_nh_half(Launcher& L, const Workspace& ws, int n, const double* mass_dev, double h, double gkT, double Q,
                  double* thermo);
 
+// virial_static.cu: the virial with its partial sums in a static device array of the library (no workspace scratch,
+// no allocation); at most kVirialStaticMaxAtoms atoms (= FLARE_VIRIAL_STATIC_MAX_ATOMS of the header)
+constexpr int64_t kVirialStaticMaxAtoms = 4194304;
+cudaError_t run_virial_static(Launcher& L, int device, const Grid& g, const Workspace& ws, int n, int mmax,
+                              double* out9);
+
 // domain.cu: selection / packing / compaction kernels of the domain decomposition (all sizes on the device)
 void dom_select(Launcher& L, const Workspace& ws, const DomSel& s, int n_bound, int* list_lo, int* list_hi,
                 int* list_stay, int cap);

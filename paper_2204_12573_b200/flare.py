@@ -32,11 +32,12 @@ EXPORTS = (
     "flare_set_state", "flare_set_state_host", "flare_set_forces", "flare_set_forces_host", "flare_step", "flare_get_state", "flare_get_state_host",
     "flare_get_neighbors", "flare_get_descriptors", "flare_get_groups", "flare_get_rows", "flare_get_timings", "flare_kernel_launches",
     "flare_last_error",
-    "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_analyze",
+    "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_virial_static", "flare_analyze",
     "flare_domain_begin", "flare_domain_migrate_pack", "flare_domain_migrate_unpack", "flare_domain_border_pack",
     "flare_domain_border_unpack", "flare_domain_commit", "flare_domain_forward_pack", "flare_domain_forward_unpack",
     "flare_domain_signal", "flare_domain_get_tags",
 )
+VIRIAL_STATIC_MAX_ATOMS = 4194304  # FLARE_VIRIAL_STATIC_MAX_ATOMS
 MSG_HEADER, MSG_FULL_ROW, MSG_FWD_ROW = 8, 11, 9  # message layout of the domain data plane (doubles)
 
 
@@ -91,6 +92,7 @@ def load_library():
     lib.flare_get_thermostat.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
     lib.flare_set_thermostat.argtypes = [vp, dbl, dbl]
     lib.flare_get_virial.argtypes = [vp, vp]
+    lib.flare_virial_static.argtypes = [vp, vp]
     lib.flare_analyze.argtypes = [vp, dbl, i32, i32, dbl, C.POINTER(dbl), C.POINTER(i64), vp, vp]
     lib.flare_domain_begin.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, dbl]
     lib.flare_domain_migrate_pack.argtypes = [vp, i32, dbl, dbl, dbl, dbl, vp, vp, i64]
@@ -300,6 +302,16 @@ class Flare:
         w = np.zeros(9)
         self._check(self._lib.flare_get_virial(self._ctx, _hp(w)))
         return w.reshape(3, 3)
+
+    def virial_static(self, out):
+        """Enqueue the virial of the last evaluation into `out`, a caller-owned float64 CUDA tensor of 9 elements, and
+        return it (valid after the bound stream is synchronised).  For callers that may not allocate device memory:
+        the reduction scratch is a static array inside the library (flare_virial_static in include/flare_b200.h:
+        at most VIRIAL_STATIC_MAX_ATOMS atoms, one shared array per GPU, so overlapping calls race)."""
+        if out.dtype != self._torch.float64 or out.numel() != 9 or not out.is_cuda or not out.is_contiguous():
+            raise ValueError("out must be a contiguous float64 CUDA tensor with 9 elements")
+        self._check(self._lib.flare_virial_static(self._ctx, C.c_void_p(out.data_ptr())))
+        return out
 
     def analyze(self, threshold: float = 0.0, species_a: int = 0, species_b: int = 0, r_coord: float = 1.0,
                 uncertainty: bool = True, coordination: bool = True):
