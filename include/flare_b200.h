@@ -53,7 +53,9 @@ enum {
     FLARE_ERR_CUDA = -6,               /* CUDA runtime error; message in flare_last_error */
     FLARE_ERR_NONFINITE = -7,          /* NaN/Inf met in positions, or produced in an energy, force or variance */
     FLARE_ERR_UNSUPPORTED = -8,        /* (n_max, l_max) outside the compiled range */
-    FLARE_ERR_NOT_BOUND = -9           /* call needs flare_bind / flare_set_state first */
+    FLARE_ERR_NOT_BOUND = -9,          /* call needs flare_bind / flare_set_state first */
+    FLARE_ERR_HALO_EXCEEDED = -10      /* domain decomposition: an atom moved further since the last rebuild than the
+                                          ghost shell covers (flare_domain_set_limit); forces since then are suspect */
 };
 
 /* Options (flare_set_option / flare_get_option).  Set them BEFORE flare_workspace_bytes/flare_bind. */
@@ -269,7 +271,10 @@ int flare_analyze(flare_ctx* ctx, double unc_threshold, int species_a, int speci
 
 /* Start domain mode: the first n_owned atoms of the state become pos / vel (may be NULL = 0) / types / tags (global
    atom ids, they travel with the atoms), all DEVICE pointers, in the local frame `box`, `pbc` (host).  A displacement
-   of any atom by trigger_displacement (Angstrom) since the last rebuild raises the rebuild signal (0: always raised). */
+   of any atom by trigger_displacement (Angstrom) since the last rebuild raises the rebuild signal (0: always raised).
+   If the call fails the context is left as it was.  While domain mode is active the whole-system calls
+   (flare_compute*, flare_set_state*) are refused with FLARE_ERR_INVALID_ARG -- the context works on its local atoms,
+   not on flare_bind's n_atoms; flare_bind ends domain mode. */
 int flare_domain_begin(flare_ctx* ctx, int64_t n_owned, const double* pos, const double* vel, const int32_t* types,
                        const int64_t* tags, const double box[9], const int pbc[3], double trigger_displacement);
 
@@ -278,7 +283,10 @@ int flare_domain_begin(flare_ctx* ctx, int64_t n_owned, const double* pos, const
    ghosts. */
 int flare_domain_migrate_pack(flare_ctx* ctx, int axis, double lo_bound, double hi_bound, double shift_lo,
                               double shift_hi, double* msg_lo, double* msg_hi, int64_t cap_rows);
-/* Append the atoms of the two received messages (either may be NULL) to the owned set. */
+/* Append the atoms of the two received messages (either may be NULL) to the owned set.  cap_rows is the capacity the
+   messages were allocated for: a header count outside [0, cap_rows] (a peer built with another capacity, a stale
+   buffer) is clamped to it and raises FLARE_ERR_WORKSPACE_TOO_SMALL at the next flare_check / flare_domain_commit;
+   nothing is read beyond the message.  The same holds for flare_domain_border_unpack. */
 int flare_domain_migrate_unpack(flare_ctx* ctx, const double* msg_lo_in, const double* msg_hi_in, int64_t cap_rows);
 
 /* Phase 0 or 1: local atoms (owned, plus the ghosts of phase 0 in phase 1) with coordinate[axis] in [lo_a, lo_b)
@@ -302,6 +310,22 @@ int flare_domain_forward_unpack(flare_ctx* ctx, int phase, const double* msg_lo_
 /* Copy the rebuild signal (0 / non-zero) of the last evaluation to a DEVICE int32: all-reduce it (MAX) over the ranks
    and rebuild when it is set.  Raised when an atom has moved trigger_displacement since the last rebuild. */
 int flare_domain_signal(flare_ctx* ctx, int32_t* flag_out);
+
+/* Copy the device-side error bits raised by the work enqueued so far (0 = none; what flare_check would turn into an
+   error code) to a DEVICE int32, without synchronising and without clearing them.  A rank that hits an error would
+   otherwise be the only one to know: reduce this (MAX) over the ranks together with the rebuild signal, and when the
+   result is non-zero let EVERY rank call flare_check and stop, instead of leaving the peers blocked in an exchange. */
+int flare_domain_status(flare_ctx* ctx, int32_t* status_out);
+
+/* Guard of the ghost shell.  The rebuild that the signal asks for happens a few steps later (the flag is all-reduced
+   and read with a lag), and until then the old shell is in use: it is complete only while no atom has moved more than
+   half the halo skin since the last rebuild.  With max_displacement > 0 (Angstrom; it must exceed the trigger
+   displacement) the kernel that tracks the displacements raises FLARE_ERR_HALO_EXCEEDED -- reported by the next
+   flare_check / flare_domain_commit -- as soon as an atom has moved that far: owned atoms may have been missing
+   dE_j/dr_jk terms since then, so the run should stop or restart from a checkpoint with a wider skin, a shorter lag or
+   a smaller time step.  0 switches the guard off (the default after flare_domain_begin and flare_bind).  Like the
+   signal it needs the candidate list (FLARE_OPT_SKIN_MILLI_ANGSTROM > 0).  Call after flare_domain_begin. */
+int flare_domain_set_limit(flare_ctx* ctx, double max_displacement);
 
 /* Global ids of the local atoms (owned first) -> DEVICE int64 [n_atoms]. */
 int flare_domain_get_tags(flare_ctx* ctx, int64_t* tags_out);

@@ -18,6 +18,7 @@ constexpr int kFlagNonFinite = 2;        // a position is NaN/Inf
 constexpr int kFlagBadType = 4;          // a species index outside 0..S-1 (stored as 0 so that indexing stays in bounds)
 constexpr int kFlagNonFiniteResult = 8;  // an energy, force or variance came out NaN/Inf
 constexpr int kFlagDomainOverflow = 16;  // domain decomposition: a message, a send list or the bound capacity is too small
+constexpr int kFlagHaloExceeded = 32;    // domain decomposition: an atom has moved further since the last rebuild than the ghost shell covers
 
 // One atom in cell-sorted order: wrapped position, species, index in the caller's order.
 struct __align__(32) AtomS {

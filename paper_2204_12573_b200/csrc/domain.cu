@@ -155,11 +155,21 @@ __global__ void k_dom_pack_full(const int* __restrict__ list, const int* __restr
 }
 
 // full rows of a message -> slots [base, base + count) of the state, base = dom[kDomNLocal] (bumped by k_dom_bump)
-__global__ void k_dom_append(const double* __restrict__ msg, const int* __restrict__ dom, int n_cap,
+// The header comes from a peer: a count that is negative, not finite or above the capacity both sides agreed on
+// (another build, a stale buffer) must not drive reads past the end of the message -- clamp and flag.
+__device__ __forceinline__ int dom_msg_rows(const double* __restrict__ msg, int cap_rows, bool* bad) {
+    const double h = msg[0];
+    *bad = !(h >= 0.0 && h <= (double)cap_rows);
+    return *bad ? (h > 0.0 ? cap_rows : 0) : (int)h;  // NaN fails both comparisons: bad, 0 rows
+}
+
+__global__ void k_dom_append(const double* __restrict__ msg, int cap_rows, const int* __restrict__ dom, int n_cap,
                              double* __restrict__ x, double* __restrict__ v, double* __restrict__ f,
                              int* __restrict__ types, long long* __restrict__ tag, int* __restrict__ flags) {
     const int base = dom[kDomNLocal];
-    int cnt = (int)msg[0];
+    bool bad;
+    int cnt = dom_msg_rows(msg, cap_rows, &bad);
+    if (bad && blockIdx.x == 0 && threadIdx.x == 0) atomicOr(flags, kFlagDomainOverflow);
     if (base + cnt > n_cap) {
         cnt = max(0, n_cap - base);
         if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(flags, kFlagDomainOverflow);
@@ -175,10 +185,12 @@ __global__ void k_dom_append(const double* __restrict__ msg, const int* __restri
 }
 
 // after k_dom_append: record where the rows went and move the end of the local set (and of the owned set for arrivals)
-__global__ void k_dom_bump(const double* __restrict__ msg, int* __restrict__ dom, int n_cap, int slot, int owned) {
+__global__ void k_dom_bump(const double* __restrict__ msg, int cap_rows, int* __restrict__ dom, int n_cap, int slot,
+                           int owned) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const int base = dom[kDomNLocal];
-    const int cnt = max(0, min((int)msg[0], n_cap - base));
+    bool bad;
+    const int cnt = max(0, min(dom_msg_rows(msg, cap_rows, &bad), n_cap - base));
     if (slot >= 0) { dom[kDomRecvOff + slot] = base; dom[kDomRecvCnt + slot] = cnt; }
     dom[kDomNLocal] = base + cnt;
     if (owned) dom[kDomNOwned] = base + cnt;
@@ -270,9 +282,9 @@ void dom_pack_full(Launcher& L, const Workspace& ws, const int* list, int cnt_sl
 }
 
 void dom_append(Launcher& L, const Workspace& ws, const double* msg, int n_cap, int max_rows, int slot, bool owned) {
-    L.launch(k_dom_append, dim3(dom_grid(max_rows)), dim3(256), 0, msg, (const int*)ws.dom, n_cap, ws.x, ws.v, ws.f,
-             ws.types, ws.tag, ws.flags);
-    L.launch(k_dom_bump, dim3(1), dim3(32), 0, msg, ws.dom, n_cap, slot, owned ? 1 : 0);
+    L.launch(k_dom_append, dim3(dom_grid(max_rows)), dim3(256), 0, msg, max_rows, (const int*)ws.dom, n_cap, ws.x, ws.v,
+             ws.f, ws.types, ws.tag, ws.flags);
+    L.launch(k_dom_bump, dim3(1), dim3(32), 0, msg, max_rows, ws.dom, n_cap, slot, owned ? 1 : 0);
 }
 
 void dom_compact_stay(Launcher& L, const Workspace& ws, const int* list_stay, int n_bound) {

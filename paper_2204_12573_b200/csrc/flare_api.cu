@@ -67,6 +67,7 @@ struct flare_ctx {
     // domain decomposition (flare_domain_*): host mirrors of the device counters after flare_domain_commit
     bool dom_active = false;
     double dom_trigger = 0.0;       // displacement since the last rebuild that raises the rebuild signal
+    double dom_limit = 0.0;         // displacement since the last rebuild that is an error (0: not checked)
     double dom_shift[4][3]{};       // frame shift of the send lists x-lo, x-hi, y-lo, y-hi
     int dom_send[4]{}, dom_recv_cnt[4]{}, dom_recv_off[4]{};
     int64_t dom_n_owned = 0;
@@ -452,7 +453,8 @@ int evaluate(flare_ctx* c, Launcher& L, const double* pos, const int* types, dou
     {
         PhaseScope ps(c, FLARE_PHASE_NEIGHBOR);
         build_neighbors(L, c->grid, c->bs, c->ws, n, pos, types, c->mmax, c->sparse, c->n_groups, eff_skin(c),
-                        c->list_valid, c->dom_active ? c->dom_trigger : 0.0);
+                        c->list_valid, c->dom_active ? c->dom_trigger : 0.0,
+                        c->dom_active ? c->dom_limit : 0.0);
         if (eff_skin(c) > 0.0) c->list_valid = true;
         // group sizes of this evaluation -> pinned host memory, read (without waiting) when the NEXT evaluation is enqueued
         if (c->h_group_start && !c->capturing && L.err == cudaSuccess)
@@ -488,6 +490,19 @@ int evaluate(flare_ctx* c, Launcher& L, const double* pos, const int* types, dou
 int need_bound(flare_ctx* c) {
     if (!c) return FLARE_ERR_INVALID_ARG;
     if (c->n < 0) return fail(c, FLARE_ERR_NOT_BOUND, "flare_bind has not been called");
+    return FLARE_OK;
+}
+
+// Calls that take whole-system arrays sized by flare_bind's n_atoms.  In domain mode the context works on the local
+// atoms (owned + ghosts, fewer than the bound capacity, in the rank's open frame) and tracks displacements against
+// the last domain rebuild: a plain call would silently evaluate a truncated system with the caller's arrays read at
+// the wrong length.  Refuse it; flare_bind ends domain mode.
+int need_plain(flare_ctx* c, const char* what) {
+    int rc = need_bound(c);
+    if (rc) return rc;
+    if (c->dom_active)
+        return fail(c, FLARE_ERR_INVALID_ARG, std::string(what) + ": the context is in domain mode (flare_domain_begin); "
+                    "call flare_bind again to return to plain whole-system calls");
     return FLARE_OK;
 }
 
@@ -667,6 +682,7 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->n = c->n_cap = n_atoms;
     c->dom_active = false;
+    c->dom_limit = 0.0;
     c->dom_list_cap = (int)(std::max<int64_t>(n_atoms, 1) / 2 + 1024);
     c->state_set = c->forces_valid = c->var_valid = false;
     c->have_grid = false;
@@ -682,7 +698,7 @@ int flare_bind(flare_ctx* c, int64_t n_atoms, void* workspace, size_t bytes, voi
 
 int flare_compute(flare_ctx* c, const double* pos, const int32_t* types, const double box[9], const int pbc[3],
                   double* e_out, double* f_out, double* var_out) {
-    int rc = need_bound(c);
+    int rc = need_plain(c, "flare_compute");
     if (rc) return rc;
     if (c->n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
     FLARE_CUDA(c, cudaSetDevice(c->device));
@@ -708,6 +724,8 @@ int flare_check(flare_ctx* c) {
     }
     if (flags[0] & kFlagDomainOverflow)
         return fail(c, FLARE_ERR_WORKSPACE_TOO_SMALL, "domain decomposition: a message buffer, a send list or the bound capacity is too small (or a peer sent a message of another step)");
+    if (flags[0] & kFlagHaloExceeded)
+        return fail(c, FLARE_ERR_HALO_EXCEEDED, "domain decomposition: an atom has moved further since the last rebuild than flare_domain_set_limit allows; the ghost shell may have missed neighbours of owned atoms since then (widen the halo skin, lower the signal lag or the time step)");
     if (flags[0] & kFlagBadType) return fail(c, FLARE_ERR_INVALID_ARG, "a species index is outside 0..S-1");
     if (flags[0] & kFlagNonFinite) return fail(c, FLARE_ERR_NONFINITE, "non-finite position");
     if (flags[0] & kFlagNeighborOverflow)
@@ -719,7 +737,7 @@ int flare_check(flare_ctx* c) {
 
 int flare_compute_host(flare_ctx* c, const double* pos, const int32_t* types, const double box[9], const int pbc[3],
                        double* e_out, double* f_out, double* var_out) {
-    int rc = need_bound(c);
+    int rc = need_plain(c, "flare_compute_host");
     if (rc) return rc;
     const size_t n = (size_t)c->n;
     if (n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
@@ -742,7 +760,7 @@ int flare_compute_host(flare_ctx* c, const double* pos, const int32_t* types, co
 
 static int set_state_impl(flare_ctx* c, const double* pos, const double* vel, const int32_t* types,
                           const double box[9], const int pbc[3], cudaMemcpyKind kind) {
-    int rc = need_bound(c);
+    int rc = need_plain(c, "flare_set_state");
     if (rc) return rc;
     const size_t n = (size_t)c->n;
     if (n > 0 && (!pos || !types)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types is null");
@@ -937,9 +955,9 @@ int flare_domain_begin(flare_ctx* c, int64_t n_owned, const double* pos, const d
     if (n_owned > 0 && (!pos || !types || !tags)) return fail(c, FLARE_ERR_INVALID_ARG, "pos/types/tags is null");
     if (!(trigger_displacement >= 0.0)) return fail(c, FLARE_ERR_INVALID_ARG, "trigger displacement must be >= 0");
     FLARE_CUDA(c, cudaSetDevice(c->device));
-    c->n = n_owned;
     rc = setup_grid(c, box, pbc);
-    if (rc) return rc;
+    if (rc) return rc;  // the context is left as it was
+    c->n = n_owned;
     const size_t n = (size_t)n_owned;
     if (n > 0) {
         FLARE_CUDA(c, cudaMemcpyAsync(c->ws.x, pos, sizeof(double) * 3 * n, cudaMemcpyDeviceToDevice, c->stream));
@@ -955,6 +973,7 @@ int flare_domain_begin(flare_ctx* c, int64_t n_owned, const double* pos, const d
     FLARE_CUDA(c, cudaMemcpy(c->ws.dom, h, sizeof(h), cudaMemcpyHostToDevice));
     c->dom_active = true;
     c->dom_trigger = trigger_displacement;
+    c->dom_limit = 0.0;
     c->dom_n_owned = n_owned;
     for (int q = 0; q < 4; q++) c->dom_send[q] = c->dom_recv_cnt[q] = c->dom_recv_off[q] = 0;
     c->state_set = true;
@@ -997,6 +1016,7 @@ int flare_domain_migrate_pack(flare_ctx* c, int axis, double lo_bound, double hi
 int flare_domain_migrate_unpack(flare_ctx* c, const double* msg_lo_in, const double* msg_hi_in, int64_t cap_rows) {
     int rc = need_domain(c);
     if (rc) return rc;
+    if (cap_rows < 0 || cap_rows > 0x7fffffff / kDomFullRow) return fail(c, FLARE_ERR_INVALID_ARG, "bad message capacity");
     FLARE_CUDA(c, cudaSetDevice(c->device));
     Launcher L = make_launcher(c);
     if (msg_lo_in) dom_append(L, c->ws, msg_lo_in, (int)c->n_cap, (int)cap_rows, -1, true);
@@ -1035,7 +1055,8 @@ int flare_domain_border_unpack(flare_ctx* c, int phase, const double* msg_lo_in,
                                int64_t cap_rows) {
     int rc = need_domain(c);
     if (rc) return rc;
-    if (phase < 0 || phase > 1) return fail(c, FLARE_ERR_INVALID_ARG, "bad phase");
+    if (phase < 0 || phase > 1 || cap_rows < 0 || cap_rows > 0x7fffffff / kDomFullRow)
+        return fail(c, FLARE_ERR_INVALID_ARG, "bad phase or message capacity");
     FLARE_CUDA(c, cudaSetDevice(c->device));
     Launcher L = make_launcher(c);
     // an absent neighbour (null) still records an empty ghost block
@@ -1117,6 +1138,26 @@ int flare_domain_signal(flare_ctx* c, int32_t* flag_out) {
         FLARE_CUDA(c, cudaMemcpyAsync(flag_out, c->ws.dom + kDomNeed, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
     else
         FLARE_CUDA(c, cudaMemsetAsync(flag_out, 1, 1, c->stream));  // no candidate list, no displacement tracking: always
+    return FLARE_OK;
+}
+
+int flare_domain_status(flare_ctx* c, int32_t* status_out) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (!status_out) return fail(c, FLARE_ERR_INVALID_ARG, "status pointer is null");
+    FLARE_CUDA(c, cudaSetDevice(c->device));
+    FLARE_CUDA(c, cudaMemcpyAsync(status_out, c->ws.flags, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
+    return FLARE_OK;
+}
+
+int flare_domain_set_limit(flare_ctx* c, double max_displacement) {
+    int rc = need_domain(c);
+    if (rc) return rc;
+    if (!(max_displacement >= 0.0)) return fail(c, FLARE_ERR_INVALID_ARG, "the displacement limit must be >= 0");
+    if (max_displacement > 0.0 && c->dom_trigger > 0.0 && !(max_displacement > c->dom_trigger))
+        return fail(c, FLARE_ERR_INVALID_ARG, "the displacement limit must exceed the trigger displacement of flare_domain_begin");
+    if (max_displacement != c->dom_limit) drop_step_graph(c);  // a captured step has the old limit baked in
+    c->dom_limit = max_displacement;
     return FLARE_OK;
 }
 

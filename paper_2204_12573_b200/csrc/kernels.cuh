@@ -287,7 +287,8 @@ struct GroupDev {
 // order / box / types) and filter it with the exact predicate; skin = 0: rebuild everything every time.
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
                      const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid,
-                     double dom_trigger = 0.0);  // > 0: raise Workspace::dom[kDomNeed] once an atom has moved that far
+                     double dom_trigger = 0.0,  // > 0: raise Workspace::dom[kDomNeed] once an atom has moved that far
+                     double dom_limit = 0.0);   // > 0: raise kFlagHaloExceeded once an atom has moved that far
 
 // Descriptor rows [row0,row0+nrows): compact A -> ws.A, UNNORMALISED B -> bh_out (row r at (r - row0)*ld),
 // ||B||^2 -> nrm_out.  One launch per group.

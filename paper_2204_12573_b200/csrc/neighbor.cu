@@ -403,7 +403,8 @@ k_reverse_index(int n, int mmax, const int* __restrict__ nbr_cnt, const int* __r
 __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, const int* __restrict__ types,
                           const int* __restrict__ order, const AtomS* __restrict__ ref, AtomS* __restrict__ atoms,
                           int* __restrict__ gate, int* __restrict__ dmax, int* __restrict__ flags,
-                          const double* __restrict__ dom_ref, double dom_trigger2, int* __restrict__ dom_need) {
+                          const double* __restrict__ dom_ref, double dom_trigger2, double dom_limit2,
+                          int* __restrict__ dom_need) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     int my_type = -1;
     int bits = 0;
@@ -428,6 +429,9 @@ __global__ void k_refresh(Grid g, int S, int n, const double* __restrict__ pos, 
                 d2 += dd * dd;
             }
             if (!(d2 < dom_trigger2)) *dom_need = 1;  // benign race: every writer stores 1
+            // the rebuild asked for above arrives a few steps later (the signal is all-reduced and read with a lag):
+            // past dom_limit the shell no longer holds every ghost an owned atom's force needs -- an error, not a signal
+            if (!(d2 < dom_limit2)) atomicOr(flags, kFlagHaloExceeded);
         }
         AtomS a;
         a.x = p[0]; a.y = p[1]; a.z = p[2];
@@ -705,7 +709,7 @@ k_group_small(int n, int S, int sparse, int n_groups, const AtomS* __restrict__ 
 // ------------------------------------------------------------------ host-side driver of a1
 void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspace& ws, int n, const double* pos,
                      const int* types, int mmax, int sparse, int n_groups, double skin, bool list_valid,
-                     double dom_trigger) {
+                     double dom_trigger, double dom_limit) {
     if (n == 0) return;
     const int tb = 256;
     const bool use_skin = skin > 0.0;
@@ -728,8 +732,9 @@ void build_neighbors(Launcher& L, const Grid& g, const Basis& bs, const Workspac
             L.memset(ws.skin_gate + 4, 0, sizeof(int) * kMaxSpecies);  // per-species maximum displacement
             L.launch(k_refresh, dim3((n + tb - 1) / tb), dim3(tb), 0, g, bs.S, n, pos, types, (const int*)ws.order,
                      (const AtomS*)ws.ref, ws.atoms, ws.skin_gate, ws.skin_gate + 4, ws.flags,
-                     dom_trigger > 0.0 ? (const double*)ws.dom_ref : (const double*)nullptr, dom_trigger * dom_trigger,
-                     ws.dom + kDomNeed);
+                     dom_trigger > 0.0 || dom_limit > 0.0 ? (const double*)ws.dom_ref : (const double*)nullptr,
+                     dom_trigger > 0.0 ? dom_trigger * dom_trigger : HUGE_VAL,
+                     dom_limit > 0.0 ? dom_limit * dom_limit : HUGE_VAL, ws.dom + kDomNeed);
             // captured step: the rebuild chain below becomes the body of an IF node that k_gate_decide switches on,
             // so a step that keeps its list pays for none of the chain's (otherwise empty) launches
             const bool as_if = L.capturing;

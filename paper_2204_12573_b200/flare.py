@@ -20,6 +20,7 @@ ERRORS = {
     -1: "FLARE_ERR_INVALID_ARG", -2: "FLARE_ERR_BOX_TOO_SMALL", -3: "FLARE_ERR_UNSUPPORTED_BOX",
     -4: "FLARE_ERR_WORKSPACE_TOO_SMALL", -5: "FLARE_ERR_NEIGHBOR_OVERFLOW", -6: "FLARE_ERR_CUDA",
     -7: "FLARE_ERR_NONFINITE", -8: "FLARE_ERR_UNSUPPORTED", -9: "FLARE_ERR_NOT_BOUND",
+    -10: "FLARE_ERR_HALO_EXCEEDED",
 }
 OPT_MAX_NEIGHBORS, OPT_CHUNK_ATOMS, OPT_TIMING, OPT_SPECIES_SPARSE, OPT_SKIN, OPT_SKIN_REBUILDS = 1, 2, 3, 4, 5, 6
 OPT_GRAPH, OPT_GRAPH_REPLAYS = 7, 8
@@ -35,7 +36,7 @@ EXPORTS = (
     "flare_step_nvt", "flare_get_thermostat", "flare_set_thermostat", "flare_get_virial", "flare_virial_static", "flare_analyze",
     "flare_domain_begin", "flare_domain_migrate_pack", "flare_domain_migrate_unpack", "flare_domain_border_pack",
     "flare_domain_border_unpack", "flare_domain_commit", "flare_domain_forward_pack", "flare_domain_forward_unpack",
-    "flare_domain_signal", "flare_domain_get_tags",
+    "flare_domain_signal", "flare_domain_get_tags", "flare_domain_set_limit", "flare_domain_status",
 )
 VIRIAL_STATIC_MAX_ATOMS = 4194304  # FLARE_VIRIAL_STATIC_MAX_ATOMS
 MSG_HEADER, MSG_FULL_ROW, MSG_FWD_ROW = 8, 11, 9  # message layout of the domain data plane (doubles)
@@ -104,6 +105,8 @@ def load_library():
     lib.flare_domain_forward_unpack.argtypes = [vp, i32, vp, vp]
     lib.flare_domain_signal.argtypes = [vp, vp]
     lib.flare_domain_get_tags.argtypes = [vp, vp]
+    lib.flare_domain_set_limit.argtypes = [vp, dbl]
+    lib.flare_domain_status.argtypes = [vp, vp]
     _lib = lib
     return lib
 
@@ -390,6 +393,14 @@ class Flare:
 
     def domain_forward_unpack(self, phase, msg_lo_in, msg_hi_in):
         self._check(self._lib.flare_domain_forward_unpack(self._ctx, int(phase), self._msg(msg_lo_in), self._msg(msg_hi_in)))
+
+    def domain_set_limit(self, max_displacement: float):
+        """Displacement since the last domain rebuild beyond which the ghost shell is no longer trusted (an error)."""
+        self._check(self._lib.flare_domain_set_limit(self._ctx, float(max_displacement)))
+
+    def domain_status(self, status):
+        """Device-side error bits so far -> int32[1] device tensor (asynchronous, not cleared)."""
+        self._check(self._lib.flare_domain_status(self._ctx, self._dev(status, self._torch.int32, (1,))))
 
     def domain_signal(self, flag):
         self._check(self._lib.flare_domain_signal(self._ctx, self._dev(flag, self._torch.int32, (1,))))

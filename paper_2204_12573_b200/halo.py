@@ -26,7 +26,10 @@ their owner does), rebuild signal.  Membership, order and counts are stable betw
 candidate neighbour list survives.  The signal -- "some atom has moved `trigger` since the rebuild", raised on the
 device by the kernel that refreshes the candidate list -- is all-reduced (MAX) asynchronously and read `lag` steps
 later, so every rank takes the same decision without a per-step host synchronisation; the halo skin covers
-2 x trigger plus the motion of those `lag` steps (trigger = 0.35 halo_skin).
+2 x trigger plus the motion of those `lag` steps (trigger = 0.35 halo_skin).  That last part is an assumption about
+the run (time step, temperature, lag), so it is also CHECKED: the shell is complete as long as no atom has moved more
+than halo_skin / 2 since the rebuild, and the engine raises FLARE_ERR_HALO_EXCEEDED (at the next check / rebuild /
+gather) the moment one has -- the 0.15 halo_skin between trigger and limit is what the `lag` steps may use up.
 """
 from __future__ import annotations
 
@@ -39,12 +42,17 @@ import torch.distributed as dist
 MSG_HEADER, MSG_FULL_ROW, MSG_FWD_ROW = 8, 11, 9  # include/flare_b200.h: message layout (doubles)
 
 
+class PeerError(RuntimeError):
+    """Another rank's engine reported an error; this rank stops with it instead of blocking in the next exchange."""
+
+
 class Engine:
     """What the decomposition needs from a force engine: the device data plane of include/flare_b200.h."""
 
     device = torch.device("cpu")
 
     def begin(self, pos, vel, types, tags, box, pbc, trigger): raise NotImplementedError
+    def set_limit(self, max_displacement): pass            # optional guard: displacement that invalidates the ghost shell
     def migrate_pack(self, axis, lo_bound, hi_bound, shift_lo, shift_hi, msg_lo, msg_hi, cap): raise NotImplementedError
     def migrate_unpack(self, msg_lo_in, msg_hi_in, cap): raise NotImplementedError
     def border_pack(self, phase, axis, lo_a, lo_b, hi_a, hi_b, shift_lo, shift_hi, msg_lo, msg_hi, cap): raise NotImplementedError
@@ -53,7 +61,8 @@ class Engine:
     def forward_pack(self, phase, msg_lo, msg_hi): raise NotImplementedError
     def forward_unpack(self, phase, msg_lo_in, msg_hi_in): raise NotImplementedError
     def step(self, dt, n_steps, variances): raise NotImplementedError   # n_steps = 0: forces of the current positions
-    def signal(self, flag): raise NotImplementedError      # flag: int32[1] tensor on `device`
+    def signal(self, flag): raise NotImplementedError      # flag: int32[2] tensor on `device`: [0] rebuild wanted, [1] error bits
+    def check(self): raise NotImplementedError             # raise this rank's pending engine error, if any
     def owned(self, variances): raise NotImplementedError  # -> host dict(tags, pos (local frame), vel, E, F, V)
 
 
@@ -78,6 +87,8 @@ class CudaEngine(Engine):
                               box, pbc, trigger)
         self.n_owned = n
 
+    def set_limit(self, max_displacement): self.ctx.domain_set_limit(max_displacement)
+
     def migrate_pack(self, *a): self.ctx.domain_migrate_pack(*a)
     def migrate_unpack(self, *a): self.ctx.domain_migrate_unpack(*a)
     def border_pack(self, *a): self.ctx.domain_border_pack(*a)
@@ -94,7 +105,11 @@ class CudaEngine(Engine):
     def step(self, dt, n_steps, variances):
         self.ctx.step(dt, n_steps, want_variance=variances)
 
-    def signal(self, flag): self.ctx.domain_signal(flag)
+    def signal(self, flag):
+        self.ctx.domain_signal(flag[0:1])
+        self.ctx.domain_status(flag[1:2])
+
+    def check(self): self.ctx.check()
 
     def owned(self, variances):
         n = self.n_owned
@@ -109,7 +124,7 @@ class DomainDecomposition:
 
     def __init__(self, engine: Engine, box, pbc, r_cut_max: float, grid=None, axes=(0, 1), halo_skin: float = 1.2,
                  lag: int = 2, border_capacity: int | None = None, migrate_capacity: int = 8192, self_halo: bool = False,
-                 group=None, rank: int | None = None, world: int | None = None):
+                 group=None, rank: int | None = None, world: int | None = None, trigger_fraction: float = 0.35):
         self.engine = engine
         self.group = group
         # rank / world default to the process group's; given explicitly they describe a rank's geometry without one (tests)
@@ -123,8 +138,19 @@ class DomainDecomposition:
         self.L = (np.diag(b.reshape(3, 3)) if b.size == 9 else b.reshape(3)).copy()
         self.pbc = np.asarray(pbc, dtype=np.int32).reshape(3).copy()
         self.h = 2.0 * float(r_cut_max) + float(halo_skin)
-        self.trigger = 0.35 * float(halo_skin)
-        self.lag = max(1, int(lag))
+        if not halo_skin > 0.0:
+            raise ValueError("halo_skin must be > 0")
+        if not 1 <= int(lag) <= 16:
+            # the flag posted after step k is read before step k + lag: with more than a few steps in between, the margin
+            # between trigger and limit (0.15 halo_skin per atom) is used up at any temperature worth simulating
+            raise ValueError(f"lag must be between 1 and 16 steps, not {lag}")
+        if not 0.0 < trigger_fraction < 0.5:
+            raise ValueError("trigger_fraction must lie in (0, 0.5): the shell is complete up to halo_skin / 2 per atom")
+        # a fast system (hot, light atoms, long time step) wants a lower fraction: (0.5 - fraction) halo_skin is what an
+        # atom may still move between raising the signal and the rebuild, `lag` steps later
+        self.trigger = float(trigger_fraction) * float(halo_skin)
+        self.limit = 0.5 * float(halo_skin)   # beyond this the ghost shell may miss a neighbour of an owned atom: an error
+        self.lag = int(lag)
         coords = (self.rank // grid[1], self.rank % grid[1])
         # decomposed axes = exchange phases, in order
         self.phases = []
@@ -182,6 +208,8 @@ class DomainDecomposition:
             q = max(self.h / ph["w"] for ph in self.phases)
             self.border_capacity = int(1.5 * (n_all / self.world) * q * (1.0 + 2.0 * q)) + 4096
         self.engine.begin(local, vel[idx], types[idx], idx.astype(np.int64), self.local_box, self.local_pbc, self.trigger)
+        if self.phases:
+            self.engine.set_limit(self.limit)
         self.built = False
         self._flags.clear()
         return self
@@ -252,7 +280,14 @@ class DomainDecomposition:
             e.border_pack(k, ph["axis"], -inf, 2.0 * self.h, ph["w"], inf, ph["w"], -ph["w"], out_lo, out_hi, bcap)
             self._exchange(ph, out_lo, out_hi, in_lo, in_hi)
             e.border_unpack(k, in_lo, in_hi, bcap)
-        self.counts = e.commit()
+        # an overflow (message, send list, capacity) shows on the rank it happened on only: agree on the outcome before
+        # anybody walks into the next exchange alone
+        try:
+            counts, failure = e.commit(), None
+        except Exception as ex:  # noqa: BLE001 -- whatever the engine raises, the peers must hear of it
+            counts, failure = None, ex
+        self._raise_together(1 if failure is not None else 0, failure, "the domain rebuild")
+        self.counts = counts
         c = self.counts
         self._fwd = [dict(out_lo=self._new_msg(c["send"][2 * k], MSG_FWD_ROW), out_hi=self._new_msg(c["send"][2 * k + 1], MSG_FWD_ROW),
                           in_lo=self._new_msg(c["recv"][2 * k], MSG_FWD_ROW), in_hi=self._new_msg(c["recv"][2 * k + 1], MSG_FWD_ROW))
@@ -268,10 +303,24 @@ class DomainDecomposition:
             self._exchange(ph, m["out_lo"], m["out_hi"], m["in_lo"], m["in_hi"])
             self.engine.forward_unpack(k, m["in_lo"], m["in_hi"])
 
+    def _raise_together(self, status: int, failure, where: str):
+        """All ranks call this at the same point with their own status (0 = fine): if any is non-zero, every rank raises
+        -- its own error where it has one, PeerError elsewhere."""
+        worst = status
+        if self.world > 1:
+            on_host = dist.get_backend(self.group) == "gloo"
+            t = torch.tensor([status], dtype=torch.int32, device="cpu" if on_host else self.engine.device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX, group=self.group)
+            worst = int(t.item())
+        if failure is not None:
+            raise failure
+        if worst != 0:
+            raise PeerError(f"rank {self.rank}: another rank reported an engine error during {where} (status {worst:#x})")
+
     # ------------------------------------------------------------------ rebuild signal (asynchronous, lagged)
     def _post_signal(self):
         dev = self.engine.device
-        flag = torch.zeros(1, dtype=torch.int32, device=dev)
+        flag = torch.zeros(2, dtype=torch.int32, device=dev)  # [0] rebuild wanted, [1] this rank's error bits so far
         self.engine.signal(flag)
         if self.world > 1:
             if dist.get_backend(self.group) == "gloo" and dev.type != "cpu":
@@ -281,7 +330,7 @@ class DomainDecomposition:
             else:
                 dist.all_reduce(flag, op=dist.ReduceOp.MAX, group=self.group)
         if flag.is_cuda:
-            host = torch.empty(1, dtype=torch.int32, pin_memory=True)
+            host = torch.empty(2, dtype=torch.int32, pin_memory=True)
             host.copy_(flag, non_blocking=True)
             ev = torch.cuda.Event()
             ev.record()
@@ -290,12 +339,16 @@ class DomainDecomposition:
             self._flags.append((flag, None))
 
     def _signal_due(self) -> bool:
-        """The flag posted `lag` steps ago (identical on all ranks); waiting on it does not stall the GPU."""
+        """The flag posted `lag` steps ago (identical on all ranks); waiting on it does not stall the GPU.  It carries
+        the ranks' error bits too: an engine error anywhere stops every rank here, in the same step."""
         if len(self._flags) < self.lag:
             return False
         host, ev = self._flags.popleft()
         if ev is not None:
             ev.synchronize()
+        if int(host[1]) != 0:
+            self.engine.check()  # the rank(s) the error belongs to raise it with its own message
+            raise PeerError(f"rank {self.rank}: another rank reported an engine error (bits {int(host[1]):#x})")
         return bool(int(host[0]) != 0)
 
     # ------------------------------------------------------------------ the two entry points

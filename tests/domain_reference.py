@@ -9,6 +9,10 @@ KAPPA = 9.648533212331e-3
 H, FULL, FWD = 8, 11, 9
 
 
+class HaloExceeded(RuntimeError):
+    """The reference's FLARE_ERR_HALO_EXCEEDED."""
+
+
 class NumpyOracleEngine:
     device = torch.device("cpu")
 
@@ -38,6 +42,13 @@ class NumpyOracleEngine:
         self.recv_off, self.recv_cnt = [0] * 4, [0] * 4
         self.ref = None
         self.need = 0
+        self.limit = 0.0
+        self.error = 0
+
+    def set_limit(self, max_displacement):
+        """flare_domain_set_limit: a displacement of that size since the last rebuild is an error, not a signal."""
+        assert max_displacement == 0.0 or max_displacement > self.trigger
+        self.limit = float(max_displacement)
 
     def _truncate(self, n):
         self.x, self.v, self.f, self.t, self.tag = self.x[:n], self.v[:n], self.f[:n], self.t[:n], self.tag[:n]
@@ -110,7 +121,13 @@ class NumpyOracleEngine:
             self.recv_off[q], self.recv_cnt[q] = len(self.x), len(rows)
             self._append(rows)
 
+    def check(self):
+        if self.error:
+            self.error = 0
+            raise HaloExceeded("an atom has moved further since the last rebuild than the ghost shell covers")
+
     def commit(self):
+        self.check()
         n = len(self.x)
         self.E, self.V = np.zeros(n), np.zeros(n)
         self.ref = self.x.copy()
@@ -149,6 +166,8 @@ class NumpyOracleEngine:
                     d[:, k] -= L[k] * np.round(d[:, k] / L[k])
             if len(d) and np.sqrt((d * d).sum(1)).max() >= self.trigger:
                 self.need = 1
+            if self.limit > 0.0 and len(d) and np.sqrt((d * d).sum(1)).max() >= self.limit:
+                self.error |= 32  # reported like the device's flag: by signal (bits), check and commit (exception)
 
     def step(self, dt, n_steps, variances):
         if not self.forces_valid:
@@ -166,6 +185,7 @@ class NumpyOracleEngine:
 
     def signal(self, flag):
         flag[0] = 1 if (self.need or self.trigger <= 0.0) else 0
+        flag[1] = self.error
 
     def owned(self, variances):
         n = self.n_owned

@@ -93,7 +93,10 @@ def test_self_halo_long_hot_run_keeps_every_atom_and_the_energy():
     ref = one.get_state_host(variances=True)
     e_ref = ref["E"].sum() + w.kinetic_energy(ref["vel"], s.types, s.mass)
     eng = CudaEngine(flare.from_system(s, device=0), capacity=3 * s.n_atoms + 4096)
-    dd = DomainDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), grid=(1, 1), self_halo=True, halo_skin=1.5)
+    # hot atoms in a random potential are fast: raise the rebuild signal early (0.2 of the skin) so that the two steps of
+    # lag stay inside the ghost shell's guarantee, which the engine checks (FLARE_ERR_HALO_EXCEEDED otherwise)
+    dd = DomainDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), grid=(1, 1), self_halo=True, halo_skin=1.5,
+                             trigger_fraction=0.2)
     dd.scatter(s.pos, s.vel, s.types)
     dd.step(dt, n_steps, variances=True)
     got = dd.gather()
@@ -174,6 +177,103 @@ def test_data_plane_matches_the_numpy_reference_call_by_call():
     with pytest.raises(flare.FlareError) as ei:
         cuda.ctx.check()
     assert ei.value.code == -4
+
+
+def test_a_bad_message_header_is_clamped_and_reported():
+    """The row count in a message header comes from a peer.  One that is above the capacity both sides agreed on,
+    negative or not a number (a peer built with another capacity, a stale buffer) must not make the unpack kernels
+    read past the message: rows are clamped to the capacity and the error surfaces at the next check / commit."""
+    from paper_2204_12573_b200 import flare
+    from paper_2204_12573_b200.halo import MSG_FULL_ROW, MSG_HEADER, CudaEngine
+
+    s = _system()
+    n, cap = s.n_atoms, 8
+    L = np.asarray(s.box, float).reshape(3, 3).diagonal()
+    box = np.diag([L[0] + 18.0, L[1] + 18.0, L[2]]).reshape(9)
+    for header, rows_kept in ((1.0e9, cap), (float(cap + 1), cap), (-3.0, 0), (float("nan"), 0)):
+        eng = CudaEngine(flare.from_system(s, device=0), capacity=_capacity(s, 1))
+        eng.begin(s.pos + np.array([9.0, 9.0, 0.0]), s.vel, s.types, np.arange(n, dtype=np.int64), box, [0, 0, 1], 0.3)
+        bad = torch.zeros(MSG_HEADER + cap * MSG_FULL_ROW, dtype=torch.float64, device="cuda")
+        bad[0] = header
+        good = torch.zeros_like(bad)
+        eng.border_unpack(0, bad, good, cap)
+        with pytest.raises(flare.FlareError) as ei:
+            eng.commit()
+        assert ei.value.code == -4
+        assert eng.commit()["n_local"] == n + rows_kept   # the flag is cleared; the clamped count stands
+    # an in-range header raises nothing
+    eng = CudaEngine(flare.from_system(s, device=0), capacity=_capacity(s, 1))
+    eng.begin(s.pos + np.array([9.0, 9.0, 0.0]), s.vel, s.types, np.arange(n, dtype=np.int64), box, [0, 0, 1], 0.3)
+    ok = torch.zeros(MSG_HEADER + cap * MSG_FULL_ROW, dtype=torch.float64, device="cuda")
+    ok[0] = float(cap)
+    eng.border_unpack(0, ok, torch.zeros_like(ok), cap)
+    assert eng.commit()["n_local"] == n + cap
+
+
+def test_an_outrun_ghost_shell_is_an_error_not_a_wrong_force():
+    """A thin halo skin whose rebuild signal is read eight steps late: hot H atoms move more than half the skin before
+    the rebuild arrives, so the shell's guarantee (every ghost an owned atom's force needs is present) no longer holds.
+    The displacement kernel flags it and the run stops with FLARE_ERR_HALO_EXCEEDED instead of integrating on."""
+    from paper_2204_12573_b200 import flare
+    from paper_2204_12573_b200.halo import CudaEngine, DomainDecomposition
+
+    s = _system()
+    s.vel = w.maxwell_velocities(np.random.default_rng(5), s.types, s.mass, 1500.0)
+    eng = CudaEngine(flare.from_system(s, device=0), capacity=_capacity(s, 1))
+    dd = DomainDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), grid=(1, 1), self_halo=True, halo_skin=0.3, lag=8)
+    dd.scatter(s.pos, s.vel, s.types)
+    with pytest.raises(flare.FlareError) as ei:
+        dd.step(1.0, 30)
+        eng.ctx.check()
+    assert ei.value.code == -10 and "ghost shell" in str(ei.value)
+    # the same run with the default skin and lag stays inside the guarantee
+    eng = CudaEngine(flare.from_system(s, device=0), capacity=_capacity(s, 1))
+    dd = DomainDecomposition(eng, s.box, s.pbc, float(np.max(s.r_cut)), grid=(1, 1), self_halo=True)
+    dd.scatter(s.pos, s.vel, s.types)
+    dd.step(0.5, 30)
+    eng.ctx.check()
+    # the limit must lie above the trigger; 0 switches the guard off
+    with pytest.raises(flare.FlareError) as ei:
+        eng.ctx.domain_set_limit(0.5 * dd.trigger)
+    assert ei.value.code == -1
+    eng.ctx.domain_set_limit(0.0)
+
+
+def test_plain_calls_are_refused_in_domain_mode_until_rebind():
+    """In domain mode the context works on its local atoms (fewer than the bound capacity): whole-system calls are
+    refused instead of silently evaluating a truncated system; flare_bind returns the context to plain use.  A
+    flare_domain_begin that fails (bad box) leaves the context as it was."""
+    from paper_2204_12573_b200 import flare
+
+    s = _system()
+    n = s.n_atoms
+    ctx = flare.from_system(s).bind(n)
+    pos = torch.as_tensor(s.pos, dtype=torch.float64, device="cuda")
+    types = torch.as_tensor(s.types, dtype=torch.int32, device="cuda")
+    e0, f0, _ = ctx.compute(pos, types, s.box, s.pbc)
+    half = n // 2
+    tags = torch.arange(half, dtype=torch.int64, device="cuda")
+    tri = np.array(s.box, dtype=np.float64).reshape(3, 3).copy()
+    tri[0, 1] = 1.0
+    with pytest.raises(flare.FlareError) as ei:   # non-orthorhombic: refused, and the context stays plain
+        ctx.domain_begin(half, pos[:half].contiguous(), None, types[:half].contiguous(), tags, tri.reshape(9), s.pbc, 0.3)
+    assert ei.value.code == -3
+    ctx.n_atoms = n
+    e1, f1, _ = ctx.compute(pos, types, s.box, s.pbc)
+    assert torch.equal(e0, e1) and torch.equal(f0, f1)
+    ctx.domain_begin(half, pos[:half].contiguous(), None, types[:half].contiguous(), tags, s.box, s.pbc, 0.3)
+    ctx.domain_commit()
+    ctx.n_atoms = n
+    for call in (lambda: ctx.compute(pos, types, s.box, s.pbc),
+                 lambda: ctx.compute_host(s.pos, s.types, s.box, s.pbc),
+                 lambda: ctx.set_state(s.pos, s.vel, s.types, s.box, s.pbc),
+                 lambda: ctx.set_state(pos, None, types, s.box, s.pbc)):
+        with pytest.raises(flare.FlareError) as ei:
+            call()
+        assert ei.value.code == -1 and "domain mode" in str(ei.value)
+    ctx.bind(n)
+    e2, f2, _ = ctx.compute(pos, types, s.box, s.pbc)
+    assert torch.equal(e0, e2) and torch.equal(f0, f2)
 
 
 def _worker(rank, world, grid, port, n_steps, dt, q):

@@ -46,7 +46,10 @@ def _worker(rank, world, grid, port, n_steps, dt, q):
         flare_oracle.set_num_threads(2)
         pos, vel, types, box, pbc, beta, sigma = make_system()
         eng = NumpyOracleEngine(flare_oracle, MASS, N_MAX, L_MAX, RC, beta, sigma)
-        dd = DomainDecomposition(eng, box, pbc, RC.max(), grid=grid, halo_skin=HALO_SKIN).scatter(pos, vel, types)
+        # 2500 K, 1.5 amu, dt = 1 fs: the fastest atoms do 0.2 A per step, so the signal is raised early enough
+        # (0.25 of the skin) for the two steps of lag to stay inside the shell's guarantee (checked by the engine)
+        dd = DomainDecomposition(eng, box, pbc, RC.max(), grid=grid, halo_skin=HALO_SKIN,
+                                 trigger_fraction=0.25).scatter(pos, vel, types)
         own0 = set(eng.tag[:eng.n_owned].tolist())
         dd.compute(variances=True)
         first = dd.gather()
@@ -101,6 +104,56 @@ def test_domain_decomposition_matches_the_undivided_system(oracle, world, grid):
     assert evaluations == world * (n_steps + 1)
 
 
+def _failing_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from domain_reference import HaloExceeded, NumpyOracleEngine
+        from oracle import flare_oracle
+        from paper_2204_12573_b200.halo import DomainDecomposition, PeerError
+
+        flare_oracle.set_num_threads(2)
+        pos, vel, types, box, pbc, beta, sigma = make_system()
+        if rank != 0:
+            vel = vel * np.where(pos[:, :1] < 0.5 * box[0], 1.0, 0.05)  # the atoms of the other ranks' half barely move
+        eng = NumpyOracleEngine(flare_oracle, MASS, N_MAX, L_MAX, RC, beta, sigma)
+        # a thin skin read six steps late: the fast atoms leave the shell's guarantee long before the rebuild arrives
+        dd = DomainDecomposition(eng, box, pbc, RC.max(), grid=(world, 1), halo_skin=0.8, lag=6).scatter(pos, vel, types)
+        steps = 0
+        try:
+            for _ in range(14):
+                dd.step(1.0, 1)
+                steps += 1
+            q.put((rank, "no error", steps))
+        except (HaloExceeded, PeerError) as ex:
+            q.put((rank, type(ex).__name__, steps))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_an_engine_error_on_one_rank_stops_every_rank_in_the_same_step():
+    """an error used to surface on the rank it happened on only, leaving its peers blocked in the next
+    exchange until the backend's timeout.  The ranks' error bits now ride with the lagged rebuild signal (all-reduce
+    MAX), so all of them stop in the same step -- the owner with its own error, the others with PeerError -- and the
+    ghost-shell guard (an atom moved more than halo_skin / 2 since the rebuild) is what raises it here."""
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_failing_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    kinds = [g[1] for g in got]
+    assert "no error" not in kinds, got
+    assert "HaloExceeded" in kinds, got
+    assert got[0][2] == got[1][2], f"the ranks stopped in different steps: {got}"
+    assert 6 <= got[0][2] < 14
+
+
 def test_geometry_checks():
     from paper_2204_12573_b200.halo import DomainDecomposition, Engine
 
@@ -108,8 +161,12 @@ def test_geometry_checks():
     dd = DomainDecomposition(Engine(), np.diag([20.0, 10.0, 10.0]).reshape(9), [1, 1, 0], 3.0)
     assert dd.world == 1 and dd.local_pbc.tolist() == [1, 1, 0] and dd.local_L.tolist() == [20.0, 10.0, 10.0]
     assert dd.phases == [] and dd.h == pytest.approx(7.2) and dd.trigger == pytest.approx(0.42)
+    assert dd.limit == pytest.approx(0.6)  # the shell is complete up to half the skin per atom
     with pytest.raises(ValueError):
         DomainDecomposition(Engine(), np.diag([20.0, 10.0, 10.0]).reshape(9), [1, 1, 0], 3.0, grid=(2, 1))
+    for bad in (dict(lag=0), dict(lag=17), dict(trigger_fraction=0.5), dict(trigger_fraction=0.0), dict(halo_skin=0.0)):
+        with pytest.raises(ValueError):
+            DomainDecomposition(Engine(), np.diag([20.0, 10.0, 10.0]).reshape(9), [1, 1, 0], 3.0, **bad)
 
 
 def test_process_grid_geometry_4x2():
