@@ -74,7 +74,8 @@ enum {
     FLARE_OPT_SKIN_REBUILDS = 6,  /* read-only (flare_get_option, synchronises): candidate-list rebuilds since flare_bind */
     FLARE_OPT_GRAPH = 7,          /* CUDA-graph replay of the MD step in flare_step / flare_step_nvt (small systems are bound by launch
                                     latency: one step of 256 atoms is ~30 tiny kernels).  -1 (default): automatic, for
-                                    n_atoms <= 200 000; 0: never; 1: always.  The first step of a run (and the step after a
+                                    n_atoms <= 200 000 outside domain mode (there every ghost rebuild would force a
+                                    re-capture); 0: never; 1: always.  The first step of a run (and the step after a
                                     re-bind, an option change or a new box) is launched plainly, the next one is captured
                                     -- with the candidate-list rebuild chain as a conditional IF node that a device-side
                                     decision switches on -- and later steps replay the graph on the bound stream.

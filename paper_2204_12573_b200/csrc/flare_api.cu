@@ -831,6 +831,9 @@ static int enqueue_md_step(flare_ctx* c, Launcher& L, double dt_fs, double* var,
 static bool graph_wanted(const flare_ctx* c) {
     if (c->graph_broken || c->graph_opt == 0 || c->n <= 0) return false;
     if (c->graph_opt == 1) return true;
+    // domain mode: every ghost rebuild (each ~10-20 steps) changes the atom count and drops the graph, and a re-capture
+    // plus cudaGraphInstantiate costs more than the launch latency saved over so few replays -- plain launches unless asked
+    if (c->dom_active) return false;
     return c->n <= 200000;  // automatic: above this a step keeps the GPU busy for longer than its launches take
 }
 

@@ -183,6 +183,7 @@ class DomainDecomposition:
         self.rebuilds = 0
         self.bytes_sent = 0
         self._flags = collections.deque()
+        self._ring, self._ring_pos = None, 0  # lag + 1 signal slots (device flag, pinned copy, event), allocated once
         self._fwd = None
         self._rb = None
 
@@ -320,7 +321,15 @@ class DomainDecomposition:
     # ------------------------------------------------------------------ rebuild signal (asynchronous, lagged)
     def _post_signal(self):
         dev = self.engine.device
-        flag = torch.zeros(2, dtype=torch.int32, device=dev)  # [0] rebuild wanted, [1] this rank's error bits so far
+        if self._ring is None:
+            # at most `lag` signals are in flight (one is read before the next is posted): lag + 1 slots never collide
+            cuda = dev.type == "cuda"
+            self._ring = [(torch.zeros(2, dtype=torch.int32, device=dev),
+                           torch.empty(2, dtype=torch.int32, pin_memory=True) if cuda else None,
+                           torch.cuda.Event() if cuda else None) for _ in range(self.lag + 1)]
+        flag, pinned, ev = self._ring[self._ring_pos % len(self._ring)]
+        self._ring_pos += 1
+        flag.zero_()  # [0] rebuild wanted, [1] this rank's error bits so far
         self.engine.signal(flag)
         if self.world > 1:
             if dist.get_backend(self.group) == "gloo" and dev.type != "cpu":
@@ -330,13 +339,11 @@ class DomainDecomposition:
             else:
                 dist.all_reduce(flag, op=dist.ReduceOp.MAX, group=self.group)
         if flag.is_cuda:
-            host = torch.empty(2, dtype=torch.int32, pin_memory=True)
-            host.copy_(flag, non_blocking=True)
-            ev = torch.cuda.Event()
+            pinned.copy_(flag, non_blocking=True)
             ev.record()
-            self._flags.append((host, ev))
+            self._flags.append((pinned, ev))
         else:
-            self._flags.append((flag, None))
+            self._flags.append((flag.clone(), None))  # the slot is reused lag + 1 steps from now
 
     def _signal_due(self) -> bool:
         """The flag posted `lag` steps ago (identical on all ranks); waiting on it does not stall the GPU.  It carries
