@@ -54,8 +54,10 @@ def _compare(s, first, last, ref_first, ref_last):
     assert np.abs(last["E"] - ref_last["E"]).max() < 1e-9
 
 
-def test_self_halo_on_one_gpu_matches_the_periodic_context():
-    """World size 1, but x and y go through the whole data path (the rank's ghosts are its own periodic images)."""
+def test_self_halo_on_one_gpu_matches_the_periodic_context(oracle):
+    """World size 1, but x and y go through the whole data path (the rank's ghosts are its own periodic images).
+    The first evaluation is compared with the ORACLE on the undivided system directly (not only through the
+    undivided CUDA context), at the parity tolerances."""
     from paper_2204_12573_b200 import flare
     from paper_2204_12573_b200.halo import CudaEngine, DomainDecomposition
 
@@ -73,6 +75,10 @@ def test_self_halo_on_one_gpu_matches_the_periodic_context():
     eng.ctx.check()
     ref_first, ref_last = _reference_run(s, dt, n_steps)
     _compare(s, first, last, ref_first, ref_last)
+    E, F, V = oracle.compute(s.pos, s.types, s.box, s.pbc, s.n_max, s.l_max, s.r_cut, s.beta, s.sigma)
+    assert np.all(np.abs(first["E"] - E) <= 1e-12 + 1e-10 * np.abs(E))
+    assert np.all(np.abs(first["F"] - F) <= 1e-12 + 1e-10 * np.abs(F))
+    assert np.all(np.abs(first["V"] - V) <= 1e-15 + 1e-10 * np.abs(V))
     assert 2 <= dd.rebuilds < n_steps // 3, dd.rebuilds
     # the candidate list is rebuilt with the ghost shell, not every step
     assert eng.ctx.get_option(OPT_SKIN_REBUILDS) <= dd.rebuilds + 2
