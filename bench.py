@@ -420,8 +420,10 @@ def sweep_entries(args, local, peaks, t_start):
     # default for small systems) and, for the per-phase kernel timeline, on plain launches
     plan = [("c1", True, 400, 20, None), ("c1", True, 200, 20, 0), ("c2", True, 200, 20, None), ("c2", True, 100, 20, 0)]
     if args.sweep == "full":
-        plan += [("c5a", True, 6, 3, None), ("c5a", False, 6, 3, None), ("c5b", True, 4, 3, None),
-                 ("c5b", False, 4, 3, None), ("c5c", True, 3, 3, None), ("c5c", False, 3, 3, None), ("c4", True, 4, 3, None)]
+        # enough timed steps that the window holds the candidate-list rebuilds a production run pays for (one per
+        # ~10 steps at 500 K, dt 0.5 fs; `skin_rebuilds_in_window` says how many fell in)
+        plan += [("c5a", True, 20, 3, None), ("c5a", False, 20, 3, None), ("c5b", True, 20, 3, None),
+                 ("c5b", False, 20, 3, None), ("c5c", True, 12, 3, None), ("c5c", False, 12, 3, None), ("c4", True, 12, 3, None)]
     cache = {}
     for name, var, steps, warm, graph in plan:
         if time.perf_counter() - t_start > args.sweep_budget:
@@ -463,6 +465,13 @@ def sweep_entries(args, local, peaks, t_start):
                      "chunk_atoms": ctx.get_option(2), "workspace_bytes_per_atom": ctx.workspace_bytes(s.n_atoms) / s.n_atoms}
             if name in ("c1", "c2"):
                 entry["us_per_step"] = res["ms_per_step"] * 1e3
+            if any(ph.values()) and (name in _C5 or name == "c4"):
+                # the same per-kernel fractions as the headline's roofline_kernels: config 5 is the one meant to show
+                # the shift from the ALU kernels to the quadratic forms as P grows
+                kr, _ = kernel_rooflines(ctx, s, res, var, peaks, steps)
+                entry["roofline_kernels"] = [{"kernel": k["kernel"], "bound": k["bound"], "ms_per_step": k["ms_per_step"],
+                                              "achieved": k["achieved"], "peak": k["peak"], "unit": k["unit"],
+                                              "frac": k["frac"]} for k in kr]
             out.append(entry)
             ctx.close()
             del ctx

@@ -62,8 +62,9 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 template <int WARPS> struct QfCfg {
     static constexpr int BM = 16 * WARPS;
     static constexpr int THREADS = 32 * WARPS;
-    static constexpr int STAGES = WARPS == 8 ? 4 : 3;
-    static constexpr int MINB = WARPS == 8 ? 1 : 2;
+    static_assert(WARPS == 4, "only the 4-warp tile is built (the 8-warp, one-CTA-per-SM variant of round 1 was slower)");
+    static constexpr int STAGES = 3;
+    static constexpr int MINB = 2;
 };
 
 template <int NB, int WARPS>
@@ -509,7 +510,10 @@ __global__ void __launch_bounds__(kQrWarps * 32 * (3 - H), 1) k_qform_res(QrArgs
     }
 }
 
-constexpr int kQrH = 1;  // rows per warp block / 8
+// rows per warp block / 8.  The kernel is written for H = 1 or 2 (H = 2 halves the matrix reads from shared memory per
+// row but needs 8 instead of 16 warps' worth of registers per warp); H = 1 was faster at every K <= 144 and is the only
+// value instantiated -- the h-loops in the kernel unroll to one pass
+constexpr int kQrH = 1;
 
 template <int K16>
 static void launch_qform_res(Launcher& L, const QrArgs& a, int sm_count) {
