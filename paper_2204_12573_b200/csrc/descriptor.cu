@@ -293,6 +293,7 @@ void run_descriptors(Launcher& L, const Grid& g, const Basis& bs, const YNorm& y
 #define FLARE_CASE(LM)                                                                                   \
     case LM:                                                                                             \
         if (bs.n_max <= 8) launch_descriptor<LM, 8>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A);       \
+        else if (bs.n_max <= 10) launch_descriptor<LM, 10>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A); \
         else if (bs.n_max <= 12) launch_descriptor<LM, 12>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A); \
         else launch_descriptor<LM, 16>(L, g, bs, yn, ws, mmax, gr, bh_out, ld, nrm_out, write_A);                    \
         break;

@@ -395,6 +395,7 @@ void run_backprop(Launcher& L, const Grid& g, const Basis& bs, const YNorm& yn, 
 #define FLARE_CASE(LM)                                                                                        \
     case LM:                                                                                                  \
         if (bs.n_max <= 8) launch_backprop<LM, 8>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);       \
+        else if (bs.n_max <= 10) launch_backprop<LM, 10>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance); \
         else if (bs.n_max <= 12) launch_backprop<LM, 12>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance); \
         else launch_backprop<LM, 16>(L, g, bs, yn, ws, mmax, gr, ld, chunk_cap, max_ntn, want_variance);                    \
         break;
