@@ -133,3 +133,24 @@ def test_slab_geometry_is_fcc111():
     bulk = (pos[:, 2] > 1.0) & (pos[:, 2] < z_top - 1.0)
     assert np.allclose(d[bulk, 1:13], nn, atol=1e-9)
     assert np.allclose(d[~bulk, 1:10], nn, atol=1e-9) and np.all(d[~bulk, 10] > nn + 0.5)
+
+
+def test_static_scratch_entry_point_constants_and_no_allocation_calls():
+    """flare_virial_static (for callers that may not allocate): the limit in the header, in the binding and in the kernel
+    file agree, and neither its translation unit nor its entry point names an allocating CUDA call."""
+    from paper_2204_12573_b200 import flare
+
+    header = open(os.path.join(ROOT, "include", "flare_b200.h")).read()
+    limit = int(re.search(r"#define\s+FLARE_VIRIAL_STATIC_MAX_ATOMS\s+(\d+)", header).group(1))
+    assert limit == flare.VIRIAL_STATIC_MAX_ATOMS == 2048 * 2048
+    csrc = os.path.join(ROOT, "paper_2204_12573_b200", "csrc")
+    unit = open(os.path.join(csrc, "virial_static.cu")).read()
+    code = "\n".join(line.split("//")[0] for line in unit.splitlines())  # comments may name the calls it avoids
+    assert re.search(r"static\s+__device__\s+__align__\(256\)\s+double\s+g_virial_rows\[", code)
+    assert "cudaGetSymbolAddress" in code
+    api = open(os.path.join(csrc, "flare_api.cu")).read()
+    body = api[api.index("int flare_virial_static("):]
+    body = body[:body.index("\n}\n")]
+    for text in (code, body):
+        for call in ("cudaMalloc", "cudaFree", "cudaMallocAsync", "cudaHostAlloc", "cub::", "thrust::"):
+            assert call not in text, call
